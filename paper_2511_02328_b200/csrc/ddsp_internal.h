@@ -1,0 +1,66 @@
+// ddsp_internal.h -- plan object and kernel launchers shared by the translation units of libddsp.
+// Product code: nothing under oracle/ is included or linked here.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <vector>
+
+#include "../../include/ddsp.h"
+
+// Geometry of the shared-memory tiled kernels for one plan.  Filled by
+// ddsp_tiled_plan(); all device tables are owned by the plan.
+struct ddsp_tiled {
+    bool ok = false;       // the tiled kernel can run this plan
+    int variant = 0;       // index into the compiled (B_dm, T) instantiations
+    int bdm = 0;           // DM trials per CTA tile
+    int tile_t = 0;        // output samples per CTA tile (on the downsampled grid)
+    int nblk = 0;          // number of DM blocks = ceil(ndm / bdm)
+    int64_t ntile_t = 0;   // number of time tiles = ceil(nsamp_out / tile_t)
+    int chunk_c = 0;       // channels staged per pipeline stage
+    int nstage = 0;        // pipeline depth
+    int row_stride = 0;    // bytes of shared memory per staged channel row (one phase copy)
+    int smem_bytes = 0;    // dynamic shared memory per CTA
+    int nchunk = 0;        // chunks per tile = ceil(nchan_unmasked / chunk_c)
+    // device tables
+    int32_t* d_base = nullptr;    // [nblk][nch_pad]  first delay of the block per listed channel
+    uint32_t* d_off = nullptr;    // [nblk][nch_pad][bdm] packed shared-memory offsets per (channel, trial)
+    int32_t* d_rows = nullptr;    // [ndm_pad] output row of each sorted trial (-1 = padding)
+    int nch_pad = 0;              // nchan_unmasked rounded up to chunk_c
+};
+
+struct ddsp_plan {
+    // problem
+    int nchan = 0, ndm = 0, ds = 1, in_dtype = DDSP_IN_U8;
+    double f_top = 0, chan_bw = 0, tsamp = 0;
+    int64_t nsamp = 0, nsamp_ds = 0, nsamp_out = 0, dmax = 0;
+    int64_t in_pitch = 0, out_pitch = 0;
+    std::vector<double> dm;          // copy of dm_list
+    std::vector<uint8_t> mask;       // copy of chan_mask (all zero if NULL)
+    std::vector<int32_t> delays;     // host, [ndm][nchan], dm_list order
+    std::vector<int32_t> chan_list;  // unmasked channels, ascending
+    std::vector<int32_t> order;      // trial indices sorted by (DM, index)
+    // device
+    int device = 0;
+    int sm_count = 0;
+    int smem_optin = 0;
+    int32_t* d_delays = nullptr;     // [ndm][nchan]
+    int32_t* d_chan_list = nullptr;  // [nchan_unmasked]
+    ddsp_tiled tiled;
+    int kernel_req = DDSP_KERNEL_AUTO;
+    int kernel = DDSP_KERNEL_DIRECT;
+    mutable int last_cuda = 0;
+    // staging buffers of ddsp_execute_host
+    void* d_stage_in = nullptr;
+    void* d_stage_out = nullptr;
+};
+
+// ddsp_direct.cu
+cudaError_t ddsp_launch_direct(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);
+
+// ddsp_tiled.cu
+// Host-side geometry + tables; returns DDSP_OK (with p->tiled.ok possibly false = unsupported) or an error.
+int ddsp_tiled_plan(ddsp_plan* p);
+void ddsp_tiled_free(ddsp_plan* p);
+cudaError_t ddsp_launch_tiled(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);

@@ -1,0 +1,237 @@
+// ddsp_plan.cpp -- C ABI of libddsp (include/ddsp.h): plan creation (delay table in double, mask
+// compaction, DM ordering), execute dispatch, host-buffer execute, destroy.
+//
+// The delay table follows PAPER.md:95-97 (Eq. 4) and PAPER.md:121 (Eq. 5) with the readings of
+// K = 4.148808e3 s MHz^2, reference = centre of channel 0 (top of band),
+// floor(x + 0.5) rounding, tsamp_ds = ds * tsamp, all in IEEE double on the host.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <numeric>
+
+#include "ddsp_internal.h"
+
+namespace {
+
+const double kDispersionConstant = 4.148808e3;  // s MHz^2 pc^-1 cm^3 (units: DESIGN.md R1)
+
+int note_cuda(const ddsp_plan* p, cudaError_t e) {
+    if (e == cudaSuccess) return DDSP_OK;
+    if (p) p->last_cuda = (int)e;
+    (void)cudaGetLastError();  // clear the sticky-less error state of this thread
+    return e == cudaErrorMemoryAllocation ? DDSP_ERR_ALLOC : DDSP_ERR_CUDA;
+}
+
+size_t elem_size_in(const ddsp_plan* p) { return p->in_dtype == DDSP_IN_U8 ? 1 : 4; }
+
+void resolve_kernel(ddsp_plan* p) {
+    if (p->kernel_req == DDSP_KERNEL_AUTO)
+        p->kernel = p->tiled.ok ? DDSP_KERNEL_TILED : DDSP_KERNEL_DIRECT;
+    else
+        p->kernel = p->kernel_req;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ddsp_version(void) { return "ddsp 0.1 (sm_100a)"; }
+
+const char* ddsp_strerror(int code) {
+    switch (code) {
+        case DDSP_OK: return "ok";
+        case DDSP_ERR_INVALID_ARG: return "invalid argument";
+        case DDSP_ERR_NO_OUTPUT: return "no output: ceil(nsamp/downsample) <= maximum delay";
+        case DDSP_ERR_UNSUPPORTED: return "unsupported";
+        case DDSP_ERR_ALLOC: return "allocation failed";
+        case DDSP_ERR_CUDA: return "CUDA error";
+        default: return "unknown error code";
+    }
+}
+
+int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, double tsamp,
+                     int64_t nsamp, const double* dm_list, int ndm, int downsample,
+                     const uint8_t* chan_mask, int in_dtype) {
+    if (!plan) return DDSP_ERR_INVALID_ARG;
+    *plan = nullptr;
+    if (nchan < 1 || ndm < 1 || downsample < 1 || nsamp < 1 || !dm_list) return DDSP_ERR_INVALID_ARG;
+    if (!(chan_bw < 0.0) || !(tsamp > 0.0) || !std::isfinite(f_top) || !std::isfinite(chan_bw) ||
+        !std::isfinite(tsamp))
+        return DDSP_ERR_INVALID_ARG;
+    if (!(f_top + (double)(nchan - 1) * chan_bw > 0.0)) return DDSP_ERR_INVALID_ARG;
+    if (in_dtype != DDSP_IN_U8 && in_dtype != DDSP_IN_F32) return DDSP_ERR_INVALID_ARG;
+    for (int i = 0; i < ndm; ++i)
+        if (!std::isfinite(dm_list[i]) || dm_list[i] < 0.0) return DDSP_ERR_INVALID_ARG;
+    if ((int64_t)ndm * nchan > ((int64_t)1 << 31) - 1) return DDSP_ERR_UNSUPPORTED;
+
+    ddsp_plan* p = new (std::nothrow) ddsp_plan;
+    if (!p) return DDSP_ERR_ALLOC;
+    int rc = DDSP_OK;
+    try {
+        p->nchan = nchan; p->ndm = ndm; p->ds = downsample; p->in_dtype = in_dtype;
+        p->f_top = f_top; p->chan_bw = chan_bw; p->tsamp = tsamp; p->nsamp = nsamp;
+        p->nsamp_ds = (nsamp + downsample - 1) / downsample;
+        p->dm.assign(dm_list, dm_list + ndm);
+        p->mask.assign((size_t)nchan, 0);
+        if (chan_mask)
+            for (int c = 0; c < nchan; ++c) p->mask[c] = chan_mask[c] ? 1 : 0;
+        for (int c = 0; c < nchan; ++c)
+            if (!p->mask[c]) p->chan_list.push_back(c);
+
+        // A1/A2: channel frequencies and the delay table, in double, in this literal order.
+        const double tsamp_ds = (double)downsample * tsamp;
+        std::vector<double> chan_term((size_t)nchan);
+        const double inv_top = 1.0 / (f_top * f_top);
+        for (int c = 0; c < nchan; ++c) {
+            const double f = f_top + (double)c * chan_bw;
+            chan_term[c] = 1.0 / (f * f) - inv_top;
+        }
+        p->delays.resize((size_t)ndm * nchan);
+        int64_t dmax = 0;
+        bool overflow = false;
+        for (int i = 0; i < ndm; ++i) {
+            const double kdm = kDispersionConstant * dm_list[i];
+            int32_t* row = &p->delays[(size_t)i * nchan];
+            for (int c = 0; c < nchan; ++c) {
+                const double v = std::floor((kdm * chan_term[c]) / tsamp_ds + 0.5);
+                if (!(v < 2147483647.0)) { overflow = true; break; }
+                row[c] = (int32_t)v;
+                if (row[c] > dmax) dmax = row[c];
+            }
+            if (overflow) break;
+        }
+        if (overflow) {
+            rc = DDSP_ERR_NO_OUTPUT;
+        } else {
+            p->dmax = dmax;
+            p->nsamp_out = p->nsamp_ds - dmax;  // PAPER.md:228 (truncate; R5)
+            if (p->nsamp_out <= 0) rc = DDSP_ERR_NO_OUTPUT;
+        }
+        if (rc == DDSP_OK) {
+            p->in_pitch = nsamp;
+            p->out_pitch = p->nsamp_out;
+            p->order.resize((size_t)ndm);
+            std::iota(p->order.begin(), p->order.end(), 0);
+            std::stable_sort(p->order.begin(), p->order.end(),
+                             [&](int a, int b) { return p->dm[a] < p->dm[b]; });
+        }
+    } catch (const std::bad_alloc&) {
+        rc = DDSP_ERR_ALLOC;
+    }
+    if (rc != DDSP_OK) { delete p; return rc; }
+
+    // device side.  Without a usable CUDA device the plan is host-only (device = -1): the getters and
+    // ddsp_plan_get_delays work, ddsp_execute fails with DDSP_ERR_CUDA.  There is no CPU fallback.
+    cudaError_t e = cudaGetDevice(&p->device);
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        p->device = -1;
+        p->last_cuda = (int)e;
+    } else {
+        cudaDeviceProp prop;
+        e = cudaGetDeviceProperties(&prop, p->device);
+        if (e == cudaSuccess) {
+            p->sm_count = prop.multiProcessorCount;
+            p->smem_optin = (int)prop.sharedMemPerBlockOptin;
+            e = cudaMalloc((void**)&p->d_delays, p->delays.size() * sizeof(int32_t));
+        }
+        if (e == cudaSuccess)
+            e = cudaMemcpy(p->d_delays, p->delays.data(), p->delays.size() * sizeof(int32_t),
+                           cudaMemcpyHostToDevice);
+        if (e == cudaSuccess && !p->chan_list.empty()) {
+            e = cudaMalloc((void**)&p->d_chan_list, p->chan_list.size() * sizeof(int32_t));
+            if (e == cudaSuccess)
+                e = cudaMemcpy(p->d_chan_list, p->chan_list.data(),
+                               p->chan_list.size() * sizeof(int32_t), cudaMemcpyHostToDevice);
+        }
+        if (e != cudaSuccess) {
+            rc = note_cuda(nullptr, e);
+            ddsp_plan_destroy(p);
+            return rc;
+        }
+    }
+    rc = ddsp_tiled_plan(p);
+    if (rc != DDSP_OK) { ddsp_plan_destroy(p); return rc; }
+    resolve_kernel(p);
+    *plan = p;
+    return DDSP_OK;
+}
+
+int ddsp_plan_set_pitch(ddsp_plan* p, int64_t in_pitch, int64_t out_pitch) {
+    if (!p || in_pitch < p->nsamp || out_pitch < p->nsamp_out) return DDSP_ERR_INVALID_ARG;
+    p->in_pitch = in_pitch;
+    p->out_pitch = out_pitch;
+    if (p->d_stage_in) { cudaFree(p->d_stage_in); p->d_stage_in = nullptr; }
+    if (p->d_stage_out) { cudaFree(p->d_stage_out); p->d_stage_out = nullptr; }
+    return DDSP_OK;
+}
+
+int ddsp_plan_set_kernel(ddsp_plan* p, int kernel) {
+    if (!p) return DDSP_ERR_INVALID_ARG;
+    if (kernel != DDSP_KERNEL_AUTO && kernel != DDSP_KERNEL_DIRECT && kernel != DDSP_KERNEL_TILED)
+        return DDSP_ERR_INVALID_ARG;
+    if (kernel == DDSP_KERNEL_TILED && !p->tiled.ok) return DDSP_ERR_UNSUPPORTED;
+    p->kernel_req = kernel;
+    resolve_kernel(p);
+    return DDSP_OK;
+}
+
+int64_t ddsp_plan_nsamp_out(const ddsp_plan* p) { return p ? p->nsamp_out : -1; }
+int64_t ddsp_plan_max_delay(const ddsp_plan* p) { return p ? p->dmax : -1; }
+int ddsp_plan_nchan_unmasked(const ddsp_plan* p) { return p ? (int)p->chan_list.size() : -1; }
+int ddsp_plan_kernel(const ddsp_plan* p) { return p ? p->kernel : -1; }
+int ddsp_plan_launches_per_execute(const ddsp_plan* p) { return p ? 1 : -1; }
+int ddsp_last_cuda_error(const ddsp_plan* p) { return p ? p->last_cuda : 0; }
+
+int ddsp_plan_get_delays(const ddsp_plan* p, int32_t* host_out) {
+    if (!p || !host_out) return DDSP_ERR_INVALID_ARG;
+    std::memcpy(host_out, p->delays.data(), p->delays.size() * sizeof(int32_t));
+    return DDSP_OK;
+}
+
+int ddsp_execute(const ddsp_plan* p, const void* d_in, void* d_out, void* cuda_stream) {
+    if (!p || !d_in || !d_out) return DDSP_ERR_INVALID_ARG;
+    if (p->device < 0) return DDSP_ERR_CUDA;  // host-only plan: no device, no fallback
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    cudaError_t e;
+    if (p->kernel == DDSP_KERNEL_TILED)
+        e = ddsp_launch_tiled(p, d_in, d_out, s);
+    else
+        e = ddsp_launch_direct(p, d_in, d_out, s);
+    return note_cuda(p, e);
+}
+
+int ddsp_execute_host(ddsp_plan* p, const void* h_in, void* h_out, void* cuda_stream) {
+    if (!p || !h_in || !h_out) return DDSP_ERR_INVALID_ARG;
+    if (p->device < 0) return DDSP_ERR_CUDA;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t in_bytes = (size_t)p->nchan * (size_t)p->in_pitch * elem_size_in(p);
+    const size_t out_bytes = (size_t)p->ndm * (size_t)p->out_pitch * 4;
+    cudaError_t e = cudaSuccess;
+    if (!p->d_stage_in) e = cudaMalloc(&p->d_stage_in, in_bytes);
+    if (e == cudaSuccess && !p->d_stage_out) e = cudaMalloc(&p->d_stage_out, out_bytes);
+    if (e != cudaSuccess) return note_cuda(p, e);
+    e = cudaMemcpyAsync(p->d_stage_in, h_in, in_bytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return note_cuda(p, e);
+    int rc = ddsp_execute(p, p->d_stage_in, p->d_stage_out, cuda_stream);
+    if (rc != DDSP_OK) return rc;
+    // Only the valid columns need to come back, but rows are pitch-strided on both sides.
+    e = cudaMemcpy2DAsync(h_out, (size_t)p->out_pitch * 4, p->d_stage_out, (size_t)p->out_pitch * 4,
+                          (size_t)p->nsamp_out * 4, (size_t)p->ndm, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    return note_cuda(p, e);
+}
+
+int ddsp_plan_destroy(ddsp_plan* p) {
+    if (!p) return DDSP_OK;
+    ddsp_tiled_free(p);
+    if (p->d_delays) cudaFree(p->d_delays);
+    if (p->d_chan_list) cudaFree(p->d_chan_list);
+    if (p->d_stage_in) cudaFree(p->d_stage_in);
+    if (p->d_stage_out) cudaFree(p->d_stage_out);
+    delete p;
+    return DDSP_OK;
+}
+
+}  // extern "C"

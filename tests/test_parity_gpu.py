@@ -1,0 +1,253 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+uint8 input: bit-exact uint32 sums.  float32 input: |g - o| <= 1e-5 |o| per element against the
+fp32 sequential oracle (north_star tolerance; R9), plus the order-independent check against
+the double-accumulated sum.  Expected values come from oracle/ only.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2511_02328_b200 import binding, build, synth
+
+from _util import (assert_f32_close, assert_u32_equal, crop, make_input, oracle_geometry, run_plan,
+                   sample_rows, to_host)
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [binding.DDSP_KERNEL_DIRECT, binding.DDSP_KERNEL_TILED]
+KNAME = {binding.DDSP_KERNEL_DIRECT: "direct", binding.DDSP_KERNEL_TILED: "tiled"}
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _built():
+    build.build()
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    binding.lib()
+
+
+def _set_kernel(plan, kernel):
+    try:
+        plan.set_kernel(kernel)
+    except binding.DdspError as e:
+        if e.code == binding.DDSP_ERR_UNSUPPORTED:
+            pytest.skip("kernel %s does not support this plan" % KNAME[kernel])
+        raise
+    assert plan.kernel == kernel
+
+
+def _compare(oracle, wl, plan, x, out, rows=None, t_lo=0, t_hi=None, what=""):
+    xh = x.cpu().numpy()
+    t_hi = plan.nsamp_out if t_hi is None else t_hi
+    got = to_host(out, plan, rows, t_lo, t_hi)
+    want, nout, dmax = oracle.dedisperse(xh, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, nsamp=wl.nsamp,
+                                         downsample=wl.downsample, mask=wl.mask, rows=rows,
+                                         t_lo=t_lo, t_hi=t_hi)
+    assert nout == plan.nsamp_out and dmax == plan.max_delay
+    if wl.dtype == "u8":
+        assert_u32_equal(got, want, what)
+    else:
+        want64, _, _ = oracle.dedisperse(xh, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, nsamp=wl.nsamp,
+                                         downsample=wl.downsample, mask=wl.mask, rows=rows,
+                                         t_lo=t_lo, t_hi=t_hi, acc64=True)
+        assert_f32_close(got, want, want64, what)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_tiny_full(oracle, kernel):
+    """BASELINE.json configs[0], every output element."""
+    wl = synth.config("tiny")
+    x = make_input(oracle, wl, "cuda")
+    with binding.plan_for(wl) as plan:
+        _set_kernel(plan, kernel)
+        out = run_plan(plan, x)
+        _compare(oracle, wl, plan, x, out, what="tiny/" + KNAME[kernel])
+        # the injected pulse (DM 100, t_p = 4096, width 3, amp 40) peaks in row 100 at its arrival time
+        row = to_host(out, plan, [100])[0].astype(np.int64)
+        assert 4096 <= int(row.argmax()) < 4099
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+@pytest.mark.parametrize("name,extra,nrows", [("fast", 9000, 40), ("wide", 5000, 40),
+                                               ("lowfreq", 6000, 40), ("rfids", 7001, 40)])
+def test_cropped_configs(oracle, name, extra, nrows, kernel):
+    """configs[1..4] with the full channel count and DM list, cropped in time: all columns of a row
+    sample (block edges, first/last, random) -- several time tiles and a ragged tail."""
+    wl = crop(oracle, synth.config(name), extra)
+    pitch = synth.round_up(wl.nsamp, 128)
+    x = make_input(oracle, wl, "cuda", pitch=pitch)
+    with binding.plan_for(wl) as plan:
+        plan.set_pitch(pitch, synth.round_up(plan.nsamp_out, 32))
+        _set_kernel(plan, kernel)
+        out = run_plan(plan, x)
+        rows = sample_rows(wl.ndm, nrows, seed=wl.seed)
+        _compare(oracle, wl, plan, x[:, :].contiguous(), out, rows=rows, what="%s-crop/%s" % (name, KNAME[kernel]))
+
+
+def _small(dtype="u8", nchan=37, nsamp=5003, ndm=23, ds=1, seed=11, dm_max=60.0, mask_frac=0.0,
+           f_top=1500.0, chan_bw=-4.0, tsamp=1e-3):
+    wl = synth.Workload("small", seed, nchan, f_top, chan_bw, tsamp, nsamp,
+                        np.linspace(0.0, dm_max, ndm), downsample=ds, dtype=dtype,
+                        mean=128.0 if dtype == "u8" else 0.0, std=30.0 if dtype == "u8" else 1.0)
+    if mask_frac > 0:
+        m = np.random.default_rng(seed).random(nchan) < mask_frac
+        wl.mask = m.astype(np.uint8)
+    return wl
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+@pytest.mark.parametrize("dtype", ["u8", "f32"])
+@pytest.mark.parametrize("ds", [1, 2, 3, 4, 8])
+def test_small_ragged(oracle, kernel, dtype, ds):
+    """Odd sizes everywhere: unaligned dense pitch, partial last bin, mask, every element compared."""
+    wl = _small(dtype=dtype, ds=ds, mask_frac=0.2, nsamp=5003 + ds)
+    x = make_input(oracle, wl, "cuda")
+    with binding.plan_for(wl) as plan:
+        _set_kernel(plan, kernel)
+        out = run_plan(plan, x)
+        _compare(oracle, wl, plan, x, out, what="small ds=%d %s" % (ds, dtype))
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_pitch_padding_untouched_and_input_unchanged(oracle, kernel):
+    wl = _small(nsamp=4100)
+    pitch = 4224
+    x = make_input(oracle, wl, "cuda", pitch=pitch)
+    x[:, wl.nsamp:] = 77                       # garbage in the input padding must never be read as data
+    x0 = x.clone()
+    with binding.plan_for(wl) as plan:
+        plan.set_pitch(pitch, plan.nsamp_out + 13)
+        _set_kernel(plan, kernel)
+        out = run_plan(plan, x, out_fill=-1234567)
+        assert torch.equal(x, x0)
+        assert bool((out[:, plan.nsamp_out:] == -1234567).all())
+        xv = x.clone()
+        xv[:, wl.nsamp:] = 0
+        got = to_host(out, plan)
+        want, _, _ = oracle.dedisperse(x.cpu().numpy(), wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list,
+                                       nsamp=wl.nsamp)
+        assert_u32_equal(got, want, "pitched")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_unsorted_duplicate_dm_list(oracle, kernel):
+    """Rows follow dm_list order whatever the order (R10); duplicates give identical rows."""
+    wl = _small(ndm=40, dm_max=90.0)
+    rng = np.random.default_rng(5)
+    dms = np.concatenate([rng.permutation(wl.dm_list), [wl.dm_list[7], wl.dm_list[7], 0.0]])
+    wl.dm_list = dms
+    x = make_input(oracle, wl, "cuda")
+    with binding.plan_for(wl) as plan:
+        _set_kernel(plan, kernel)
+        out = run_plan(plan, x)
+        _compare(oracle, wl, plan, x, out, what="unsorted")
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+@pytest.mark.parametrize("case", ["ndm1", "nchan1", "nout1", "allmasked", "onechan", "dm0only"])
+def test_degenerate(oracle, kernel, case):
+    kw = dict(ndm1=dict(ndm=1, dm_max=0.0), nchan1=dict(nchan=1), nout1=dict(), allmasked=dict(),
+              onechan=dict(), dm0only=dict(ndm=3, dm_max=0.0))[case]
+    wl = _small(**kw)
+    if case == "ndm1":
+        wl.dm_list = np.array([33.0])
+    if case == "nout1":
+        _, dmax, _ = oracle_geometry(oracle, wl)
+        wl = wl.cropped(dmax + 1)
+    if case == "allmasked":
+        wl.mask = np.ones(wl.nchan, dtype=np.uint8)
+    if case == "onechan":
+        wl.mask = np.ones(wl.nchan, dtype=np.uint8)
+        wl.mask[wl.nchan - 1] = 0
+    x = make_input(oracle, wl, "cuda")
+    with binding.plan_for(wl) as plan:
+        _set_kernel(plan, kernel)
+        out = run_plan(plan, x, out_fill=-1)
+        _compare(oracle, wl, plan, x, out, what=case)
+        if case == "allmasked":
+            assert not to_host(out, plan).any()
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_I10_saturation_headroom(oracle, kernel):
+    """x = 255 everywhere, downsample 4, 4096 channels: every output is 4 177 920 (16-bit lanes of a
+    packed accumulator would overflow 64 times over)."""
+    wl = synth.Workload("sat", 0, 4096, 1500.0, -0.1220703125, 64e-6, 4 * 3000,
+                        np.arange(0, 41, dtype=np.float64) * 2.0, downsample=4)
+    x = torch.full((wl.nchan, wl.nsamp), 255, dtype=torch.uint8, device="cuda")
+    with binding.plan_for(wl) as plan:
+        _set_kernel(plan, kernel)
+        out = run_plan(plan, x)
+        got = to_host(out, plan)
+        assert got.min() == got.max() == 4177920
+        # and ds = 1 with the full 8-bit range: 4096 * 255
+        wl1 = synth.Workload("sat1", 0, 4096, 1500.0, -0.1220703125, 64e-6, 9000,
+                             np.arange(0, 41, dtype=np.float64) * 2.0)
+    with binding.plan_for(wl1) as plan:
+        _set_kernel(plan, kernel)
+        out = run_plan(plan, x[:, :9000].contiguous())
+        got = to_host(out, plan)
+        assert got.min() == got.max() == 4096 * 255
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_I5_masked_channels_never_read(oracle, kernel):
+    """NaN / Inf in zapped fp32 channels and 255 in zapped u8 channels cannot reach the output."""
+    for dtype in ("f32", "u8"):
+        wl = _small(dtype=dtype, mask_frac=0.3, seed=3)
+        x = make_input(oracle, wl, "cuda")
+        with binding.plan_for(wl) as plan:
+            _set_kernel(plan, kernel)
+            ref = to_host(run_plan(plan, x), plan)
+            x2 = x.clone()
+            zap = torch.as_tensor(np.flatnonzero(wl.mask), device="cuda")
+            x2[zap] = float("nan") if dtype == "f32" else 255
+            got = to_host(run_plan(plan, x2), plan)
+            assert np.array_equal(got, ref)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_I2_impulse_and_I3_shift(oracle, kernel):
+    wl = _small(nchan=64, nsamp=9000, ndm=33, dm_max=128.0)
+    table, dmax, nout = oracle_geometry(oracle, wl)
+    k, t0, amp = 20, 3000, 7
+    x = torch.zeros((wl.nchan, wl.nsamp), dtype=torch.uint8, device="cuda")
+    for c in range(wl.nchan):
+        x[c, t0 + int(table[k, c])] = amp
+    with binding.plan_for(wl) as plan:
+        _set_kernel(plan, kernel)
+        got = to_host(run_plan(plan, x), plan)
+        assert got[k, t0] == wl.nchan * amp and got.max() == wl.nchan * amp
+        shift = 129
+        xs = torch.zeros_like(x)
+        xs[:, shift:] = x[:, :-shift]
+        gs = to_host(run_plan(plan, xs), plan)
+        assert np.array_equal(gs[:, shift:], got[:, :-shift])
+
+
+def test_execute_host_matches_device(oracle):
+    wl = _small(nsamp=6000)
+    x = make_input(oracle, wl, "cuda")
+    with binding.plan_for(wl) as plan:
+        dev = to_host(run_plan(plan, x), plan)
+        xh = x.cpu().pin_memory()
+        oh = torch.empty((plan.ndm, plan.out_pitch), dtype=torch.int32).pin_memory()
+        plan.execute_host(xh, oh)
+        assert np.array_equal(oh.numpy().view(np.uint32), dev)
+
+
+def test_two_streams_concurrent(oracle):
+    wl = _small(nsamp=7000)
+    x1 = make_input(oracle, wl, "cuda")
+    x2 = torch.flip(x1, dims=[1]).contiguous()
+    with binding.plan_for(wl) as plan:
+        o1 = torch.empty((plan.ndm, plan.out_pitch), dtype=torch.int32, device="cuda")
+        o2 = torch.empty_like(o1)
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        plan.execute(x1, o1, stream=s1)
+        plan.execute(x2, o2, stream=s2)
+        torch.cuda.synchronize()
+        for xx, oo in ((x1, o1), (x2, o2)):
+            want, _, _ = oracle.dedisperse(xx.cpu().numpy(), wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list)
+            assert_u32_equal(to_host(oo, plan), want, "stream")
