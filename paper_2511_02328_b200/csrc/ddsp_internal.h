@@ -27,6 +27,7 @@ struct ddsp_tiled {
     int32_t* d_base = nullptr;    // [nblk][nch_pad]  first delay of the block per listed channel
     uint32_t* d_off = nullptr;    // [nblk][nch_pad][bdm] packed shared-memory offsets per (channel, trial)
     int32_t* d_rows = nullptr;    // [ndm_pad] output row of each sorted trial (-1 = padding)
+    int32_t* d_chan = nullptr;    // [nch_pad] channel index of each listed channel
     int nch_pad = 0;              // nchan_unmasked rounded up to chunk_c
 };
 
@@ -63,4 +64,6 @@ cudaError_t ddsp_launch_direct(const ddsp_plan* p, const void* d_in, void* d_out
 // Host-side geometry + tables; returns DDSP_OK (with p->tiled.ok possibly false = unsupported) or an error.
 int ddsp_tiled_plan(ddsp_plan* p);
 void ddsp_tiled_free(ddsp_plan* p);
+// true if this execute call meets the tiled kernel's alignment needs (16-byte base and row pitch)
+bool ddsp_tiled_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);
 cudaError_t ddsp_launch_tiled(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);

@@ -195,7 +195,11 @@ int ddsp_execute(const ddsp_plan* p, const void* d_in, void* d_out, void* cuda_s
     if (p->device < 0) return DDSP_ERR_CUDA;  // host-only plan: no device, no fallback
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e;
-    if (p->kernel == DDSP_KERNEL_TILED)
+    if (p->kernel == DDSP_KERNEL_TILED && !ddsp_tiled_can_run(p, d_in, d_out)) {
+        // unaligned buffers: correct through the direct kernel unless the tiled one was forced
+        if (p->kernel_req == DDSP_KERNEL_TILED) return DDSP_ERR_UNSUPPORTED;
+        e = ddsp_launch_direct(p, d_in, d_out, s);
+    } else if (p->kernel == DDSP_KERNEL_TILED)
         e = ddsp_launch_tiled(p, d_in, d_out, s);
     else
         e = ddsp_launch_direct(p, d_in, d_out, s);
