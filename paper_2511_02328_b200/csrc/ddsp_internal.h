@@ -15,19 +15,23 @@ struct ddsp_tiled {
     bool ok = false;       // the tiled kernel can run this plan
     int variant = 0;       // index into the compiled (B_dm, T) instantiations
     int bdm = 0;           // DM trials per CTA tile
+    int threads = 0;       // threads per CTA
     int tile_t = 0;        // output samples per CTA tile (on the downsampled grid)
     int nblk = 0;          // number of DM blocks = ceil(ndm / bdm)
     int64_t ntile_t = 0;   // number of time tiles = ceil(nsamp_out / tile_t)
-    int chunk_c = 0;       // channels staged per pipeline stage
+    int chunk_c = 0;       // channels staged per pipeline stage (a power of two)
+    int chunk_shift = 0;   // log2(chunk_c)
     int nstage = 0;        // pipeline depth
     int row_stride = 0;    // bytes of shared memory per staged channel row (one phase copy)
     int smem_bytes = 0;    // dynamic shared memory per CTA
     int nchunk = 0;        // chunks per tile = ceil(nchan_unmasked / chunk_c)
     // device tables
-    int32_t* d_base = nullptr;    // [nblk][nch_pad]  first delay of the block per listed channel
-    uint32_t* d_off = nullptr;    // [nblk][nch_pad][bdm] packed shared-memory offsets per (channel, trial)
+    int64_t* d_meta = nullptr;    // [nblk][nch_pad] row-window byte offset at t0 = 0 (needs in_pitch) | units << 48
+    uint32_t* d_off = nullptr;    // [nblk][nch_pad][bdm] shared-memory byte offsets per (channel, trial)
     int32_t* d_rows = nullptr;    // [ndm_pad] output row of each sorted trial (-1 = padding)
-    int32_t* d_chan = nullptr;    // [nch_pad] channel index of each listed channel
+    std::vector<int32_t> h_base;  // [nblk][nch_pad] 16-byte-aligned first delay of the block per listed channel
+    std::vector<uint16_t> h_nunit; // [nblk][nch_pad] 16-byte units of each row window that are needed
+    std::vector<int32_t> h_chan;  // [nch_pad] channel index of each listed channel (padding repeats the last)
     int nch_pad = 0;              // nchan_unmasked rounded up to chunk_c
 };
 
@@ -63,6 +67,7 @@ cudaError_t ddsp_launch_direct(const ddsp_plan* p, const void* d_in, void* d_out
 // ddsp_tiled.cu
 // Host-side geometry + tables; returns DDSP_OK (with p->tiled.ok possibly false = unsupported) or an error.
 int ddsp_tiled_plan(ddsp_plan* p);
+int ddsp_tiled_set_pitch(ddsp_plan* p);   // rebuilds the pitch-dependent table
 void ddsp_tiled_free(ddsp_plan* p);
 // true if this execute call meets the tiled kernel's alignment needs (16-byte base and row pitch)
 bool ddsp_tiled_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);

@@ -164,7 +164,7 @@ int ddsp_plan_set_pitch(ddsp_plan* p, int64_t in_pitch, int64_t out_pitch) {
     p->out_pitch = out_pitch;
     if (p->d_stage_in) { cudaFree(p->d_stage_in); p->d_stage_in = nullptr; }
     if (p->d_stage_out) { cudaFree(p->d_stage_out); p->d_stage_out = nullptr; }
-    return DDSP_OK;
+    return ddsp_tiled_set_pitch(p);
 }
 
 int ddsp_plan_set_kernel(ddsp_plan* p, int kernel) {

@@ -22,6 +22,7 @@
 // sequential sum (R9).  With ds > 1 the bins ((x0 + x1) + x2) + ... are formed at staging.
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <vector>
 
 #include "ddsp_internal.h"
@@ -31,24 +32,26 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 // compile-time geometry
 // ------------------------------------------------------------------------------------------------
-constexpr int kThreads = 512;          // 16 warps = 4 time slabs x 4 trial groups
-constexpr int kSlabs = 4;
-constexpr int kGroups = 4;
+constexpr int kSlabs = 4;               // time slabs of 512 samples; warps = kSlabs x trial groups
 constexpr int kWT = 4;                 // 32-bit words per thread per trial (strided by 32 lanes)
 constexpr int kTileT = kSlabs * kWT * 128;   // 2048 output samples per CTA (uint8 path)
 constexpr int kFlushEvery = 256;       // channels between flushes of the 16-bit lanes
-constexpr int kMaxUnits = 4;           // 16-byte staging units per thread per chunk
-constexpr int kMaxChunkC = 32;
+constexpr int kUnitsPerRowMax = 256;   // 16-byte units of a row window that the staging threads can cover
+
+// accumulation variants of the uint8 hot loop
+constexpr int kAccHybrid = 0;   // even lanes: LOP3 + IADD3 (two rows per add); odd lanes: PRMT + IMAD
+constexpr int kAccWide = 1;     // even lanes: LOP3 + IADD3; whole word: one IMAD.WIDE into a 64-bit sum
 
 struct TiledArgs {
     const uint8_t* in;
     uint32_t* out;
-    const int32_t* base;      // [nblk][nch_pad] 16-byte-aligned first byte of each row window (rel. to t0)
-    const uint32_t* off;      // [nblk][nch_pad][bdm] phase * row_stride + (q >> 2) * 4
+    const int64_t* meta;      // [nblk][nch_pad] bits 0..47: byte offset of the row window at t0 = 0
+                              //                  (c * in_pitch + base); bits 48..63: 16-byte units needed
+    const uint32_t* off;      // [nblk][nch_pad][bdm] byte offset inside a stage: (slot*4 + phase)*row_stride + (q>>2)*4
     const int32_t* rows;      // [nblk * bdm] output row of each sorted trial, -1 = padding
-    const int32_t* chan;      // [nch_pad] channel index of each listed channel (padding repeats the last)
-    int64_t in_pitch, out_pitch, nsamp_out, in_bytes;
-    int nlist, nch_pad, nblk, chunk_c, nchunk, row_stride, units_per_row, out_vec, in_vec;
+    int64_t out_pitch, nsamp_out, in_bytes;
+    int nlist, nch_pad, nblk, chunk_shift, nchunk, row_stride, out_vec, in_vec;
+    uint32_t one;             // 1: multiplier that routes an add through the FMA pipe (IMAD / IMAD.WIDE)
 };
 
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
@@ -56,13 +59,30 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
     return v;
 }
+__device__ __forceinline__ void lds128(uint32_t addr, uint32_t* v) {
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(addr));
+}
+// acc += v on the FMA pipe (IMAD): the ALU pipe (LOP3/PRMT/IADD3, 64 lanes/clk/SM) is the busier one
+__device__ __forceinline__ void add_fma_pipe(uint32_t& acc, uint32_t v, uint32_t one) {
+    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(acc) : "r"(v), "r"(one));
+}
+__device__ __forceinline__ void add_wide(uint64_t& acc, uint32_t v, uint32_t one) {
+    asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(v), "r"(one));
+}
 
 // ------------------------------------------------------------------------------------------------
 // uint8, ds = 1
 // ------------------------------------------------------------------------------------------------
-template <int BDM_T>   // trials per thread; BDM = kGroups * BDM_T
-__global__ void __launch_bounds__(kThreads, 1) ddsp_tiled_u8_kernel(const TiledArgs a) {
-    constexpr int BDM = kGroups * BDM_T;
+// BDM_T trials per thread, GROUPS trial groups (BDM = GROUPS * BDM_T trials per CTA, 128 * GROUPS
+// threads), MODE = accumulation variant
+template <int BDM_T, int GROUPS, int MODE>
+__global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const TiledArgs a) {
+    constexpr int BDM = GROUPS * BDM_T;
+    constexpr int kThreads = 32 * kSlabs * GROUPS;
+    constexpr int kThreadsLog2 = GROUPS == 8 ? 10 : 9;
+    static_assert(GROUPS == 4 || GROUPS == 8, "4 or 8 trial groups");
+    // 16-byte staging units per thread per chunk: chunk_c * kUnitsPerRowMax units over kThreads threads
+    constexpr int kMaxUnits = GROUPS == 8 ? 2 : 4;
     extern __shared__ __align__(16) uint8_t smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slab = warp & (kSlabs - 1), grp = warp / kSlabs;
@@ -70,41 +90,59 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_tiled_u8_kernel(const TiledA
     const int64_t tile = blockIdx.x / a.nblk;
     const int64_t t0 = tile * kTileT;
 
-    const int stage_rows_bytes = a.chunk_c * 4 * a.row_stride;
-    const int stage_bytes = stage_rows_bytes + a.chunk_c * BDM * 4;
+    const int chunk_c = 1 << a.chunk_shift;
+    const int stage_rows_bytes = chunk_c * 4 * a.row_stride;
+    const int stage_bytes = stage_rows_bytes + chunk_c * BDM * 4;
     const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
 
-    const int32_t* __restrict__ base_b = a.base + (size_t)blk * a.nch_pad;
+    const int64_t* __restrict__ meta_b = a.meta + (size_t)blk * a.nch_pad;
     const uint32_t* __restrict__ off_b = a.off + (size_t)blk * a.nch_pad * BDM;
 
-    // packed accumulators: E = samples (0,2), O = samples (1,3) of each owned word, 16-bit lanes
-    uint32_t accE[BDM_T][kWT], accO[BDM_T][kWT];
+    // packed accumulators of each owned word (4 consecutive samples s0..s3):
+    //   accE = (s0, s2) in 16-bit lanes; accO = (s1, s3) [hybrid] / accW = 64-bit sum of whole words [wide]
+    uint32_t accE[BDM_T][kWT];
+    uint32_t accO[MODE == kAccHybrid ? BDM_T : 1][kWT];
+    uint64_t accW[MODE == kAccWide ? BDM_T : 1][kWT];
 #pragma unroll
-    for (int j = 0; j < BDM_T; ++j)
+    for (int k = 0; k < kWT; ++k) {
 #pragma unroll
-        for (int k = 0; k < kWT; ++k) accE[j][k] = accO[j][k] = 0;
+        for (int j = 0; j < BDM_T; ++j) accE[j][k] = 0;
+#pragma unroll
+        for (int j = 0; j < (MODE == kAccHybrid ? BDM_T : 1); ++j) accO[j][k] = 0;
+#pragma unroll
+        for (int j = 0; j < (MODE == kAccWide ? BDM_T : 1); ++j) accW[j][k] = 0;
+    }
 
-    // staging registers: kMaxUnits x (16 bytes + the following word), and the chunk's offset table
+    // Staging: 512 / chunk_c consecutive threads serve one row slot; a thread owns the 16-byte units
+    // p0, p0 + tpr, p0 + 2 tpr, p0 + 3 tpr of that row in every chunk.
+    const int tpr_shift = kThreadsLog2 - a.chunk_shift;
+    const int srow = tid >> tpr_shift, p0 = tid & ((1 << tpr_shift) - 1), tpr = 1 << tpr_shift;
     uint4 pre[kMaxUnits];
     uint32_t nxt[kMaxUnits];
-    uint32_t ptab[2];
-    const int units_total = a.chunk_c * a.units_per_row;
-    const uint8_t* in_end = a.in + a.in_bytes;
+    uint32_t ptab = 0;
+    int64_t meta_cur, meta_nxt;
+    uint32_t live = 0;          // bit u: unit u of the chunk being prefetched is needed
 
-    auto prefetch = [&](int chunk) {
+    auto load_meta = [&](int chunk) -> int64_t {
+        return chunk < a.nchunk ? __ldg(meta_b + (chunk << a.chunk_shift) + srow) : 0;
+    };
+    auto prefetch = [&](int chunk, int64_t m) {
+        const int nunit = (int)(m >> 48);
+        const int64_t so = (m & 0xffffffffffffLL) + t0 + p0 * 16;
+        const uint8_t* src = a.in + so;
+        const int64_t room = a.in_bytes - so;       // bytes that may be read from src on
+        live = 0;
 #pragma unroll
         for (int u = 0; u < kMaxUnits; ++u) {
-            const int unit = tid + u * kThreads;
+            const int p = p0 + u * tpr;
             pre[u] = make_uint4(0, 0, 0, 0);
             nxt[u] = 0;
-            if (unit < units_total) {
-                const int r = unit / a.units_per_row, p = unit - r * a.units_per_row;
-                const int l = chunk * a.chunk_c + r;
-                const int c = __ldg(a.chan + l);
-                const uint8_t* src = a.in + (size_t)c * (size_t)a.in_pitch + (t0 + __ldg(base_b + l)) + p * 16;
+            if (p < nunit) {
+                live |= 1u << u;
+                const int64_t d = (int64_t)u * tpr * 16;
                 if (a.in_vec) {
-                    if (src + 16 <= in_end) pre[u] = __ldg(reinterpret_cast<const uint4*>(src));
-                    if (src + 20 <= in_end) nxt[u] = __ldg(reinterpret_cast<const uint32_t*>(src + 16));
+                    if (d + 16 <= room) pre[u] = __ldg(reinterpret_cast<const uint4*>(src + d));
+                    if (d + 20 <= room) nxt[u] = __ldg(reinterpret_cast<const uint32_t*>(src + d + 16));
                 } else {   // unaligned base pointer or row pitch: gather the 20 bytes one by one
                     uint32_t w[5];
 #pragma unroll
@@ -112,28 +150,24 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_tiled_u8_kernel(const TiledA
                         w[q] = 0;
 #pragma unroll
                         for (int b = 0; b < 4; ++b)
-                            if (src + q * 4 + b < in_end) w[q] |= (uint32_t)__ldg(src + q * 4 + b) << (8 * b);
+                            if (d + q * 4 + b < room) w[q] |= (uint32_t)__ldg(src + d + q * 4 + b) << (8 * b);
                     }
                     pre[u] = make_uint4(w[0], w[1], w[2], w[3]);
                     nxt[u] = w[4];
                 }
             }
         }
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const int e = tid + u * kThreads;
-            ptab[u] = (e < a.chunk_c * BDM) ? __ldg(off_b + (size_t)chunk * a.chunk_c * BDM + e) : 0u;
-        }
+        if (tid < chunk_c * BDM) ptab = __ldg(off_b + (size_t)chunk * chunk_c * BDM + tid);
     };
-
+    // Units that are not needed are not written either: whatever a stage holds there is never read
+    // by a stored output.
     auto commit = [&](int stage) {
         uint8_t* sb = smem + (size_t)stage * stage_bytes;
+        uint8_t* dst0 = sb + (size_t)(srow * 4) * a.row_stride + p0 * 16;
 #pragma unroll
         for (int u = 0; u < kMaxUnits; ++u) {
-            const int unit = tid + u * kThreads;
-            if (unit < units_total) {
-                const int r = unit / a.units_per_row, p = unit - r * a.units_per_row;
-                uint8_t* dst = sb + (size_t)(r * 4) * a.row_stride + p * 16;
+            if (live & (1u << u)) {
+                uint8_t* dst = dst0 + u * tpr * 16;
                 const uint32_t w0 = pre[u].x, w1 = pre[u].y, w2 = pre[u].z, w3 = pre[u].w, w4 = nxt[u];
                 *reinterpret_cast<uint4*>(dst) = pre[u];
                 *reinterpret_cast<uint4*>(dst + a.row_stride) =
@@ -147,27 +181,35 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_tiled_u8_kernel(const TiledA
                                __byte_perm(w2, w3, 0x6543), __byte_perm(w3, w4, 0x6543));
             }
         }
-        uint32_t* tb = reinterpret_cast<uint32_t*>(sb + stage_rows_bytes);
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            const int e = tid + u * kThreads;
-            if (e < a.chunk_c * BDM) tb[e] = ptab[u];
-        }
+        if (tid < chunk_c * BDM) reinterpret_cast<uint32_t*>(sb + stage_rows_bytes)[tid] = ptab;
     };
 
     bool first_flush = true;
     auto flush = [&]() {
-#pragma unroll
+#pragma unroll 1
         for (int j = 0; j < BDM_T; ++j) {
             const int row = __ldg(a.rows + blk * BDM + grp * BDM_T + j);
 #pragma unroll
             for (int k = 0; k < kWT; ++k) {
                 const int64_t t = t0 + slab * (kWT * 128) + k * 128 + lane * 4;
-                const uint32_t e = accE[j][k], o = accO[j][k];
-                accE[j][k] = accO[j][k] = 0;
+                uint32_t e = 0, o = 0;
+                uint64_t ws = 0;
+#pragma unroll
+                for (int jj = 0; jj < BDM_T; ++jj)      // static register indexing under a rolled loop
+                    if (jj == j) {
+                        e = accE[jj][k]; accE[jj][k] = 0;
+                        if (MODE == kAccHybrid) { o = accO[jj][k]; accO[jj][k] = 0; }
+                        if (MODE == kAccWide) { ws = accW[jj][k]; accW[jj][k] = 0; }
+                    }
                 if (row < 0 || t >= a.nsamp_out) continue;
                 uint32_t* p = a.out + (size_t)row * (size_t)a.out_pitch + t;
-                uint32_t v0 = e & 0xffffu, v1 = o & 0xffffu, v2 = e >> 16, v3 = o >> 16;
+                uint32_t v0 = e & 0xffffu, v2 = e >> 16, v1, v3;
+                if (MODE == kAccHybrid) {
+                    v1 = o & 0xffffu; v3 = o >> 16;
+                } else {   // sum(w) = B0 + 2^8 B1 + 2^16 B2 + 2^24 B3 and e = B0 + 2^16 B2
+                    const uint64_t r = ws - (uint64_t)e;
+                    v1 = (uint32_t)(r >> 8) & 0xffffu; v3 = (uint32_t)(r >> 24);
+                }
                 if (a.out_vec && t + 3 < a.nsamp_out) {
                     if (!first_flush) {
                         const uint4 old = *reinterpret_cast<const uint4*>(p);
@@ -187,48 +229,84 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_tiled_u8_kernel(const TiledA
 
     // byte offset of this thread's first word inside a phase copy (relative to the row window start)
     const uint32_t lane_off = (uint32_t)(slab * (kWT * 128) + lane * 4);
+    const uint32_t one = a.one;
 
-    prefetch(0);
+    meta_cur = load_meta(0);
+    meta_nxt = load_meta(1);
+    prefetch(0, meta_cur);
     commit(0);
     __syncthreads();
     int since_flush = 0;
     for (int chunk = 0; chunk < a.nchunk; ++chunk) {
         const int stage = chunk & 1;
         const bool more = chunk + 1 < a.nchunk;
-        if (more) prefetch(chunk + 1);
-        const int nrow = min(a.chunk_c, a.nlist - chunk * a.chunk_c);
+        meta_cur = meta_nxt;                     // arrived during the previous chunk
+        meta_nxt = load_meta(chunk + 2);
+        if (more) prefetch(chunk + 1, meta_cur);
+        const int nrow = min(chunk_c, a.nlist - (chunk << a.chunk_shift));
         if (since_flush + nrow > kFlushEvery) { flush(); since_flush = 0; }
         since_flush += nrow;
 
         const uint32_t sbase = smem_base + (uint32_t)stage * stage_bytes;
-        const uint32_t tbase = sbase + stage_rows_bytes + grp * (BDM_T * 4);
-        uint32_t rbase = sbase + lane_off;
-#pragma unroll 2
-        for (int r = 0; r < nrow; ++r) {
-            uint32_t offs[BDM_T];
+        uint32_t tptr = sbase + stage_rows_bytes + grp * (BDM_T * 4);
+        const uint32_t rbase = sbase + lane_off;
+        int r = 0;
+        for (; r + 2 <= nrow; r += 2) {          // two rows per iteration: their even lanes share one IADD3
+            uint32_t o0[BDM_T], o1[BDM_T];
 #pragma unroll
             for (int j = 0; j < BDM_T; j += 4) {
-                asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];"
-                             : "=r"(offs[j]), "=r"(offs[j + 1]), "=r"(offs[j + 2]), "=r"(offs[j + 3])
-                             : "r"(tbase + (uint32_t)(r * BDM * 4 + j * 4)));
+                lds128(tptr + (uint32_t)(j * 4), &o0[j]);
+                lds128(tptr + (uint32_t)(BDM * 4 + j * 4), &o1[j]);
             }
+            tptr += 2 * BDM * 4;
 #pragma unroll
             for (int j = 0; j < BDM_T; ++j) {
-                const uint32_t addr = rbase + offs[j];
+                const uint32_t a0 = rbase + o0[j], a1 = rbase + o1[j];
 #pragma unroll
                 for (int k = 0; k < kWT; ++k) {
-                    const uint32_t w = lds32(addr + k * 128);
-                    accE[j][k] += w & 0x00ff00ffu;
-                    accO[j][k] += __byte_perm(w, 0, 0x4341);
+                    const uint32_t w0 = lds32(a0 + k * 128), w1 = lds32(a1 + k * 128);
+                    accE[j][k] = accE[j][k] + (w0 & 0x00ff00ffu) + (w1 & 0x00ff00ffu);   // IADD3 (ALU pipe)
+                    if (MODE == kAccHybrid) {
+                        add_fma_pipe(accO[j][k], __byte_perm(w0, 0, 0x4341), one);      // IMAD  (FMA pipe)
+                        add_fma_pipe(accO[j][k], __byte_perm(w1, 0, 0x4341), one);
+                    } else {
+                        add_wide(accW[j][k], w0, one);                                  // IMAD.WIDE
+                        add_wide(accW[j][k], w1, one);
+                    }
                 }
             }
-            rbase += 4 * a.row_stride;
+        }
+        if (r < nrow) {                          // odd row count
+            uint32_t o0[BDM_T];
+#pragma unroll
+            for (int j = 0; j < BDM_T; j += 4) lds128(tptr + (uint32_t)(j * 4), &o0[j]);
+#pragma unroll
+            for (int j = 0; j < BDM_T; ++j) {
+                const uint32_t a0 = rbase + o0[j];
+#pragma unroll
+                for (int k = 0; k < kWT; ++k) {
+                    const uint32_t w0 = lds32(a0 + k * 128);
+                    accE[j][k] += w0 & 0x00ff00ffu;
+                    if (MODE == kAccHybrid) accO[j][k] += __byte_perm(w0, 0, 0x4341);
+                    else accW[j][k] += w0;
+                }
+            }
         }
         if (more) commit(stage ^ 1);
         __syncthreads();
     }
     flush();
 }
+
+typedef void (*TiledKernel)(const TiledArgs);
+struct Variant { int bdm_t; int groups; int mode; TiledKernel fn; };
+const Variant kVariants[] = {
+    {4, 8, kAccHybrid, ddsp_tiled_u8_kernel<4, 8, kAccHybrid>},   // 32 trials, 1024 threads, <= 64 registers
+    {8, 4, kAccHybrid, ddsp_tiled_u8_kernel<8, 4, kAccHybrid>},   // 32 trials, 512 threads
+    {4, 4, kAccHybrid, ddsp_tiled_u8_kernel<4, 4, kAccHybrid>},   // 16 trials, 512 threads
+    {4, 4, kAccWide, ddsp_tiled_u8_kernel<4, 4, kAccWide>},
+};
+constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
 }  // namespace
 
@@ -246,61 +324,63 @@ cudaError_t upload(T** dptr, const std::vector<T>& h) {
 
 }  // namespace
 
-int ddsp_tiled_plan(ddsp_plan* p) {
-    ddsp_tiled& g = p->tiled;
-    g.ok = false;
+// Geometry of variant v for this plan; false if its staged rows do not fit.
+static bool tiled_geometry(const ddsp_plan* p, int v, ddsp_tiled& g) {
     const int nlist = (int)p->chan_list.size();
-    if (p->in_dtype != DDSP_IN_U8 || p->ds != 1 || nlist < 1) return DDSP_OK;   // other paths: direct kernel
     const int smem_budget = (p->smem_optin > 0 ? p->smem_optin : 232448) - 1024;
-
-    // Try the wide DM block first; fall back to the narrow one when the delay spread of a block
-    // makes the staged rows too long for shared memory.
-    for (int bdm_t : {8, 4}) {
-        const int bdm = kGroups * bdm_t;
-        const int nblk = (p->ndm + bdm - 1) / bdm;
-        // spread of each block/channel and the longest row window
-        int64_t max_len = 0;
-        for (int b = 0; b < nblk; ++b) {
-            const int i0 = p->order[(size_t)b * bdm];
-            const int i1 = p->order[std::min<size_t>((size_t)b * bdm + bdm, (size_t)p->ndm) - 1];
-            for (int l = 0; l < nlist; ++l) {
-                const int c = p->chan_list[l];
-                const int64_t lo = p->delays[(size_t)i0 * p->nchan + c] & ~15;
-                const int64_t hi = p->delays[(size_t)i1 * p->nchan + c];
-                max_len = std::max<int64_t>(max_len, hi - lo);
-            }
+    const int bdm = kVariants[v].groups * kVariants[v].bdm_t;
+    const int threads = 128 * kVariants[v].groups;
+    const int nblk = (p->ndm + bdm - 1) / bdm;
+    // longest row window over all (block, channel): from the 16-byte-aligned first delay to the last
+    int64_t max_len = 0;
+    for (int b = 0; b < nblk; ++b) {
+        const int i0 = p->order[(size_t)b * bdm];
+        const int i1 = p->order[std::min<size_t>((size_t)b * bdm + bdm, (size_t)p->ndm) - 1];
+        for (int l = 0; l < nlist; ++l) {
+            const int c = p->chan_list[l];
+            const int64_t lo = p->delays[(size_t)i0 * p->nchan + c] & ~15;
+            const int64_t hi = p->delays[(size_t)i1 * p->nchan + c];
+            max_len = std::max<int64_t>(max_len, hi - lo);
         }
-        // row window: offsets up to max_len, plus T samples, plus 3 bytes of phase shift, in 16-byte units
-        const int64_t units = (max_len + kTileT + 3 + 15) / 16 + 1;
-        if (units * 16 > 60000) continue;
+    }
+    // bytes [0, max_len + T) are read; phase copy 3 of the last unit needs 3 more
+    const int64_t units = (max_len + kTileT + 3 + 15) / 16;
+    // chunk_c rows per stage, a power of two; the threads of a row slot must cover its units
+    for (int shift = 4; shift >= 1; --shift) {
+        const int chunk_c = 1 << shift;
+        if (units * chunk_c > 8 * kUnitsPerRowMax) continue;
+        if (chunk_c * bdm > threads) continue;
         const int row_stride = (int)units * 16;
-        int chunk_c = std::min(kMaxChunkC, (kMaxUnits * kThreads) / (int)units);
-        chunk_c = std::min(chunk_c, (2 * kThreads) / bdm);
-        while (chunk_c >= 2 && 2 * (chunk_c * (4 * row_stride + bdm * 4)) > smem_budget) --chunk_c;
-        if (chunk_c < 2) continue;
-        chunk_c = std::min(chunk_c, std::max(2, nlist));
-        g.variant = bdm_t == 8 ? 0 : 1;
+        const int smem = 2 * (chunk_c * (4 * row_stride + bdm * 4));
+        if (smem > smem_budget) continue;
+        g.variant = v;
         g.bdm = bdm;
+        g.threads = threads;
         g.tile_t = kTileT;
         g.nblk = nblk;
         g.ntile_t = (p->nsamp_out + kTileT - 1) / kTileT;
         g.chunk_c = chunk_c;
+        g.chunk_shift = shift;
         g.nstage = 2;
         g.row_stride = row_stride;
-        g.smem_bytes = 2 * (chunk_c * (4 * row_stride + bdm * 4));
+        g.smem_bytes = smem;
         g.nchunk = (nlist + chunk_c - 1) / chunk_c;
-        g.nch_pad = g.nchunk * chunk_c;
-        g.ok = true;
-        break;
+        g.nch_pad = (g.nchunk + 2) * chunk_c;     // the metadata prefetch looks two chunks ahead
+        return (int64_t)g.ntile_t * g.nblk <= 2147483647LL;
     }
-    if (!g.ok) return DDSP_OK;
-    if ((int64_t)g.ntile_t * g.nblk > 2147483647LL) { g.ok = false; return DDSP_OK; }
+    return false;
+}
 
-    // tables
+static int tiled_build_tables(ddsp_plan* p) {
+    ddsp_tiled& g = p->tiled;
+    const int nlist = (int)p->chan_list.size();
     const int bdm = g.bdm;
-    std::vector<int32_t> base((size_t)g.nblk * g.nch_pad), rows((size_t)g.nblk * bdm, -1), chan((size_t)g.nch_pad);
+    std::vector<int32_t> rows((size_t)g.nblk * bdm, -1);
     std::vector<uint32_t> off((size_t)g.nblk * g.nch_pad * bdm);
-    for (int l = 0; l < g.nch_pad; ++l) chan[l] = p->chan_list[std::min(l, nlist - 1)];
+    g.h_base.assign((size_t)g.nblk * g.nch_pad, 0);
+    g.h_nunit.assign((size_t)g.nblk * g.nch_pad, 0);
+    g.h_chan.assign((size_t)g.nch_pad, 0);
+    for (int l = 0; l < g.nch_pad; ++l) g.h_chan[l] = p->chan_list[std::min(l, nlist - 1)];
     for (int b = 0; b < g.nblk; ++b) {
         for (int j = 0; j < bdm; ++j) {
             const size_t s = (size_t)b * bdm + j;
@@ -308,27 +388,29 @@ int ddsp_tiled_plan(ddsp_plan* p) {
         }
         const int i0 = p->order[(size_t)b * bdm];
         for (int l = 0; l < g.nch_pad; ++l) {
-            const int c = chan[l];
+            const int c = g.h_chan[l];
+            const int slot = l % g.chunk_c;
             const int32_t lo = p->delays[(size_t)i0 * p->nchan + c] & ~15;
-            base[(size_t)b * g.nch_pad + l] = lo;
+            g.h_base[(size_t)b * g.nch_pad + l] = lo;
+            int32_t qmax = 0;
             for (int j = 0; j < bdm; ++j) {
                 const size_t s = std::min<size_t>((size_t)b * bdm + j, (size_t)p->ndm - 1);
                 const int32_t q = p->delays[(size_t)p->order[s] * p->nchan + c] - lo;
-                off[((size_t)b * g.nch_pad + l) * bdm + j] = (uint32_t)((q & 3) * g.row_stride + (q >> 2) * 4);
+                qmax = std::max(qmax, q);
+                off[((size_t)b * g.nch_pad + l) * bdm + j] =
+                    (uint32_t)((slot * 4 + (q & 3)) * g.row_stride + (q >> 2) * 4);
             }
+            const int need = (qmax + kTileT + 3 + 15) / 16;
+            g.h_nunit[(size_t)b * g.nch_pad + l] = (uint16_t)(l < nlist ? std::min(need, g.row_stride / 16) : 0);
         }
     }
     if (p->device < 0) return DDSP_OK;   // host-only plan: geometry only
-    cudaError_t e = upload(&g.d_base, base);
-    if (e == cudaSuccess) e = upload(&g.d_off, off);
+    cudaError_t e = upload(&g.d_off, off);
     if (e == cudaSuccess) e = upload(&g.d_rows, rows);
-    if (e == cudaSuccess) e = upload(&g.d_chan, chan);
-    if (e == cudaSuccess) {
-        // the attribute belongs to the function, not to a plan: always opt in to the device maximum
-        e = cudaFuncSetAttribute(ddsp_tiled_u8_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_optin);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(ddsp_tiled_u8_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_optin);
-    }
+    if (e == cudaSuccess) e = cudaMalloc((void**)&g.d_meta, g.h_base.size() * sizeof(int64_t));
+    // the attribute belongs to the function, not to a plan: always opt in to the device maximum
+    for (int v = 0; v < kNumVariants && e == cudaSuccess; ++v)
+        e = cudaFuncSetAttribute(kVariants[v].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_optin);
     if (e != cudaSuccess) {
         p->last_cuda = (int)e;
         (void)cudaGetLastError();
@@ -336,16 +418,48 @@ int ddsp_tiled_plan(ddsp_plan* p) {
         g.ok = false;
         return e == cudaErrorMemoryAllocation ? DDSP_ERR_ALLOC : DDSP_ERR_CUDA;
     }
+    return ddsp_tiled_set_pitch(p);
+}
+
+int ddsp_tiled_plan(ddsp_plan* p) {
+    ddsp_tiled& g = p->tiled;
+    g.ok = false;
+    const int nlist = (int)p->chan_list.size();
+    if (p->in_dtype != DDSP_IN_U8 || p->ds != 1 || nlist < 1) return DDSP_OK;   // other paths: direct kernel
+    // Variants in order of preference; a forced variant (DDSP_TILED_VARIANT, tuning only) comes first.
+    int forced = -1;
+    if (const char* ev = getenv("DDSP_TILED_VARIANT")) forced = atoi(ev);
+    for (int k = -1; k < kNumVariants && !g.ok; ++k) {
+        const int v = k < 0 ? forced : k;
+        if (v < 0 || v >= kNumVariants) continue;
+        g.ok = tiled_geometry(p, v, g);
+    }
+    if (!g.ok) return DDSP_OK;
+    return tiled_build_tables(p);
+}
+
+// Row-window metadata depends on the input pitch: offset = c * in_pitch + base, packed with the unit count.
+int ddsp_tiled_set_pitch(ddsp_plan* p) {
+    ddsp_tiled& g = p->tiled;
+    if (!g.ok || p->device < 0) return DDSP_OK;
+    if ((int64_t)p->nchan * p->in_pitch >= ((int64_t)1 << 47)) { g.ok = false; return DDSP_OK; }
+    std::vector<int64_t> meta(g.h_base.size());
+    for (int b = 0; b < g.nblk; ++b)
+        for (int l = 0; l < g.nch_pad; ++l) {
+            const size_t i = (size_t)b * g.nch_pad + l;
+            meta[i] = ((int64_t)g.h_chan[l] * p->in_pitch + g.h_base[i]) | ((int64_t)g.h_nunit[i] << 48);
+        }
+    cudaError_t e = cudaMemcpy(g.d_meta, meta.data(), meta.size() * sizeof(int64_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { p->last_cuda = (int)e; (void)cudaGetLastError(); return DDSP_ERR_CUDA; }
     return DDSP_OK;
 }
 
 void ddsp_tiled_free(ddsp_plan* p) {
     ddsp_tiled& g = p->tiled;
-    if (g.d_base) cudaFree(g.d_base);
+    if (g.d_meta) cudaFree(g.d_meta);
     if (g.d_off) cudaFree(g.d_off);
     if (g.d_rows) cudaFree(g.d_rows);
-    if (g.d_chan) cudaFree(g.d_chan);
-    g.d_base = nullptr; g.d_off = nullptr; g.d_rows = nullptr; g.d_chan = nullptr;
+    g.d_meta = nullptr; g.d_off = nullptr; g.d_rows = nullptr;
 }
 
 bool ddsp_tiled_can_run(const ddsp_plan* p, const void* d_in, const void* d_out) {
@@ -358,18 +472,14 @@ cudaError_t ddsp_launch_tiled(const ddsp_plan* p, const void* d_in, void* d_out,
     TiledArgs a;
     a.in = (const uint8_t*)d_in;
     a.out = (uint32_t*)d_out;
-    a.base = g.d_base; a.off = g.d_off; a.rows = g.d_rows; a.chan = g.d_chan;
-    a.in_pitch = p->in_pitch; a.out_pitch = p->out_pitch; a.nsamp_out = p->nsamp_out;
+    a.meta = g.d_meta; a.off = g.d_off; a.rows = g.d_rows;
+    a.out_pitch = p->out_pitch; a.nsamp_out = p->nsamp_out; a.one = 1u;
     a.in_bytes = (int64_t)p->nchan * p->in_pitch;
     a.nlist = (int)p->chan_list.size(); a.nch_pad = g.nch_pad; a.nblk = g.nblk;
-    a.chunk_c = g.chunk_c; a.nchunk = g.nchunk; a.row_stride = g.row_stride;
-    a.units_per_row = g.row_stride / 16;
+    a.chunk_shift = g.chunk_shift; a.nchunk = g.nchunk; a.row_stride = g.row_stride;
     a.out_vec = ((uintptr_t)d_out % 16 == 0) && (p->out_pitch % 4 == 0);
     a.in_vec = ((uintptr_t)d_in % 16 == 0) && (p->in_pitch % 16 == 0);
     const unsigned grid = (unsigned)(g.ntile_t * g.nblk);
-    if (g.variant == 0)
-        ddsp_tiled_u8_kernel<8><<<grid, kThreads, g.smem_bytes, s>>>(a);
-    else
-        ddsp_tiled_u8_kernel<4><<<grid, kThreads, g.smem_bytes, s>>>(a);
+    kVariants[g.variant].fn<<<grid, g.threads, g.smem_bytes, s>>>(a);
     return cudaGetLastError();
 }
