@@ -41,6 +41,13 @@ constexpr int kUnitsPerRowMax = 256;   // 16-byte units of a row window that the
 // accumulation variants of the uint8 hot loop
 constexpr int kAccHybrid = 0;   // even lanes: LOP3 + IADD3 (two rows per add); odd lanes: PRMT + IMAD
 constexpr int kAccWide = 1;     // even lanes: LOP3 + IADD3; whole word: one IMAD.WIDE into a 64-bit sum
+constexpr int kAccAllFma = 2;   // both lanes: extract on the ALU pipe, every add an IMAD
+constexpr int kAccAllAlu = 3;   // both lanes: extract + IADD3 (two rows per add), nothing on the FMA pipe
+// "full word" variants: accE accumulates the WHOLE word (mod 2^32), accO the odd bytes (PRMT).  At flush
+// accE - (accO << 8) = B0 + 2^16 B2 exactly (mod 2^32), so the even bytes never need extracting.
+constexpr int kAccFullP = 4;    // whole word: IADD3 (two rows per add);  odd bytes: PRMT + IMAD
+constexpr int kAccFullQ = 5;    // whole word: IMAD;                      odd bytes: PRMT + IMAD
+constexpr int kAccFullR = 6;    // whole word: IADD3;                     odd bytes: PRMT + IADD3
 
 struct TiledArgs {
     const uint8_t* in;
@@ -51,6 +58,7 @@ struct TiledArgs {
     const int32_t* rows;      // [nblk * bdm] output row of each sorted trial, -1 = padding
     int64_t out_pitch, nsamp_out, in_bytes;
     int nlist, nch_pad, nblk, chunk_shift, nchunk, row_stride, out_vec, in_vec;
+    int debug_nostage;        // tuning only: skip staging after the first chunk (wrong results)
     uint32_t one;             // 1: multiplier that routes an add through the FMA pipe (IMAD / IMAD.WIDE)
 };
 
@@ -101,14 +109,14 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
     // packed accumulators of each owned word (4 consecutive samples s0..s3):
     //   accE = (s0, s2) in 16-bit lanes; accO = (s1, s3) [hybrid] / accW = 64-bit sum of whole words [wide]
     uint32_t accE[BDM_T][kWT];
-    uint32_t accO[MODE == kAccHybrid ? BDM_T : 1][kWT];
+    uint32_t accO[MODE != kAccWide ? BDM_T : 1][kWT];
     uint64_t accW[MODE == kAccWide ? BDM_T : 1][kWT];
 #pragma unroll
     for (int k = 0; k < kWT; ++k) {
 #pragma unroll
         for (int j = 0; j < BDM_T; ++j) accE[j][k] = 0;
 #pragma unroll
-        for (int j = 0; j < (MODE == kAccHybrid ? BDM_T : 1); ++j) accO[j][k] = 0;
+        for (int j = 0; j < (MODE != kAccWide ? BDM_T : 1); ++j) accO[j][k] = 0;
 #pragma unroll
         for (int j = 0; j < (MODE == kAccWide ? BDM_T : 1); ++j) accW[j][k] = 0;
     }
@@ -198,13 +206,14 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
                 for (int jj = 0; jj < BDM_T; ++jj)      // static register indexing under a rolled loop
                     if (jj == j) {
                         e = accE[jj][k]; accE[jj][k] = 0;
-                        if (MODE == kAccHybrid) { o = accO[jj][k]; accO[jj][k] = 0; }
+                        if (MODE != kAccWide) { o = accO[jj][k]; accO[jj][k] = 0; }
                         if (MODE == kAccWide) { ws = accW[jj][k]; accW[jj][k] = 0; }
                     }
                 if (row < 0 || t >= a.nsamp_out) continue;
                 uint32_t* p = a.out + (size_t)row * (size_t)a.out_pitch + t;
+                if (MODE >= kAccFullP) e -= o << 8;     // whole-word sum -> even bytes (exact mod 2^32)
                 uint32_t v0 = e & 0xffffu, v2 = e >> 16, v1, v3;
-                if (MODE == kAccHybrid) {
+                if (MODE != kAccWide) {
                     v1 = o & 0xffffu; v3 = o >> 16;
                 } else {   // sum(w) = B0 + 2^8 B1 + 2^16 B2 + 2^24 B3 and e = B0 + 2^16 B2
                     const uint64_t r = ws - (uint64_t)e;
@@ -238,8 +247,8 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
     __syncthreads();
     int since_flush = 0;
     for (int chunk = 0; chunk < a.nchunk; ++chunk) {
-        const int stage = chunk & 1;
-        const bool more = chunk + 1 < a.nchunk;
+        const int stage = a.debug_nostage ? 0 : (chunk & 1);
+        const bool more = chunk + 1 < a.nchunk && !a.debug_nostage;
         meta_cur = meta_nxt;                     // arrived during the previous chunk
         meta_nxt = load_meta(chunk + 2);
         if (more) prefetch(chunk + 1, meta_cur);
@@ -265,10 +274,22 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
 #pragma unroll
                 for (int k = 0; k < kWT; ++k) {
                     const uint32_t w0 = lds32(a0 + k * 128), w1 = lds32(a1 + k * 128);
-                    accE[j][k] = accE[j][k] + (w0 & 0x00ff00ffu) + (w1 & 0x00ff00ffu);   // IADD3 (ALU pipe)
-                    if (MODE == kAccHybrid) {
+                    if (MODE == kAccAllFma) {
+                        add_fma_pipe(accE[j][k], w0 & 0x00ff00ffu, one);
+                        add_fma_pipe(accE[j][k], w1 & 0x00ff00ffu, one);
+                    } else if (MODE == kAccFullP || MODE == kAccFullR) {
+                        accE[j][k] = accE[j][k] + w0 + w1;
+                    } else if (MODE == kAccFullQ) {
+                        add_fma_pipe(accE[j][k], w0, one);
+                        add_fma_pipe(accE[j][k], w1, one);
+                    } else {
+                        accE[j][k] = accE[j][k] + (w0 & 0x00ff00ffu) + (w1 & 0x00ff00ffu);   // IADD3 (ALU pipe)
+                    }
+                    if (MODE == kAccHybrid || MODE == kAccAllFma || MODE == kAccFullP || MODE == kAccFullQ) {
                         add_fma_pipe(accO[j][k], __byte_perm(w0, 0, 0x4341), one);      // IMAD  (FMA pipe)
                         add_fma_pipe(accO[j][k], __byte_perm(w1, 0, 0x4341), one);
+                    } else if (MODE == kAccAllAlu || MODE == kAccFullR) {
+                        accO[j][k] = accO[j][k] + __byte_perm(w0, 0, 0x4341) + __byte_perm(w1, 0, 0x4341);
                     } else {
                         add_wide(accW[j][k], w0, one);                                  // IMAD.WIDE
                         add_wide(accW[j][k], w1, one);
@@ -286,8 +307,8 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
 #pragma unroll
                 for (int k = 0; k < kWT; ++k) {
                     const uint32_t w0 = lds32(a0 + k * 128);
-                    accE[j][k] += w0 & 0x00ff00ffu;
-                    if (MODE == kAccHybrid) accO[j][k] += __byte_perm(w0, 0, 0x4341);
+                    accE[j][k] += (MODE >= kAccFullP) ? w0 : (w0 & 0x00ff00ffu);
+                    if (MODE != kAccWide) accO[j][k] += __byte_perm(w0, 0, 0x4341);
                     else accW[j][k] += w0;
                 }
             }
@@ -305,6 +326,11 @@ const Variant kVariants[] = {
     {8, 4, kAccHybrid, ddsp_tiled_u8_kernel<8, 4, kAccHybrid>},   // 32 trials, 512 threads
     {4, 4, kAccHybrid, ddsp_tiled_u8_kernel<4, 4, kAccHybrid>},   // 16 trials, 512 threads
     {4, 4, kAccWide, ddsp_tiled_u8_kernel<4, 4, kAccWide>},
+    {8, 4, kAccAllFma, ddsp_tiled_u8_kernel<8, 4, kAccAllFma>},
+    {8, 4, kAccAllAlu, ddsp_tiled_u8_kernel<8, 4, kAccAllAlu>},
+    {8, 4, kAccFullP, ddsp_tiled_u8_kernel<8, 4, kAccFullP>},
+    {8, 4, kAccFullQ, ddsp_tiled_u8_kernel<8, 4, kAccFullQ>},
+    {8, 4, kAccFullR, ddsp_tiled_u8_kernel<8, 4, kAccFullR>},
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
@@ -474,6 +500,7 @@ cudaError_t ddsp_launch_tiled(const ddsp_plan* p, const void* d_in, void* d_out,
     a.out = (uint32_t*)d_out;
     a.meta = g.d_meta; a.off = g.d_off; a.rows = g.d_rows;
     a.out_pitch = p->out_pitch; a.nsamp_out = p->nsamp_out; a.one = 1u;
+    a.debug_nostage = getenv("DDSP_DEBUG_NOSTAGE") ? 1 : 0;
     a.in_bytes = (int64_t)p->nchan * p->in_pitch;
     a.nlist = (int)p->chan_list.size(); a.nch_pad = g.nch_pad; a.nblk = g.nblk;
     a.chunk_shift = g.chunk_shift; a.nchunk = g.nchunk; a.row_stride = g.row_stride;
