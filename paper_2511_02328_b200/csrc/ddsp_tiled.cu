@@ -333,6 +333,8 @@ const Variant kVariants[] = {
     {4, 4, kAccHybrid, ddsp_tiled_u8_kernel<4, 4, kAccHybrid>},   // 16 trials, 512 threads
     {4, 8, kAccHybrid, ddsp_tiled_u8_kernel<4, 8, kAccHybrid>},   // 32 trials, 1024 threads, <= 64 registers
     {4, 4, kAccWide, ddsp_tiled_u8_kernel<4, 4, kAccWide>},
+    {4, 8, kAccFullR, ddsp_tiled_u8_kernel<4, 8, kAccFullR>},     // 32 trials, 1024 threads
+    {4, 8, kAccFullP, ddsp_tiled_u8_kernel<4, 8, kAccFullP>},
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
