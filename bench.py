@@ -36,7 +36,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="fast", help="workload name (synth.CONFIG_NAMES); headline = fast")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "tiled"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "tiled", "ring"])
     ap.add_argument("--crop", type=int, default=0, help="debug: crop to this many output samples")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -175,7 +175,7 @@ def run_ours(args):
     in_pitch = synth.round_up(wl.nsamp, 128)
     out_pitch = synth.round_up(plan.nsamp_out, 32)
     plan.set_pitch(in_pitch, out_pitch)
-    plan.set_kernel({"auto": 0, "direct": 1, "tiled": 2}[args.kernel])
+    plan.set_kernel({"auto": 0, "direct": 1, "tiled": 2, "ring": 3}[args.kernel])
     x = synth.make_input(wl, dev, pitch=in_pitch, native_delays=library_native_delays(wl),
                          nsamp_out=plan.nsamp_out)
     out = torch.empty((plan.ndm, out_pitch), dtype=torch.int32 if wl.dtype == "u8" else torch.float32,
@@ -234,7 +234,7 @@ def run_ours(args):
                        "nchan": wl.nchan, "nchan_unmasked": plan.nchan_unmasked, "ndm": plan.ndm,
                        "nsamp": wl.nsamp, "nsamp_out": plan.nsamp_out, "tsamp_s": wl.tsamp,
                        "downsample": wl.downsample, "in_dtype": wl.dtype,
-                       "kernel": {1: "direct", 2: "tiled"}[plan.kernel],
+                       "kernel": {1: "direct", 2: "tiled", 3: "ring"}[plan.kernel],
                        "units": "one observation per GPU", "parallelism": "dp%d" % world,
                        "l2": "inputs (%.2f GB) larger than L2; no flush" % (x.numel() * x.element_size() / 1e9)},
             "x_realtime": plan.nsamp_out * wl.tsamp * wl.downsample / (t_max / args.steps),

@@ -57,7 +57,9 @@ enum {
 enum {
     DDSP_KERNEL_AUTO = 0,
     DDSP_KERNEL_DIRECT = 1, /* one thread per output element, reads global memory directly (any plan) */
-    DDSP_KERNEL_TILED = 2   /* shared-memory tiled kernel */
+    DDSP_KERNEL_TILED = 2,  /* shared-memory tiled kernel, rows staged through registers (first version) */
+    DDSP_KERNEL_RING = 3    /* shared-memory tiled kernel, rows staged by the copy engine into an mbarrier ring
+                               (DESIGN.md section 6); needs a 16-byte aligned input base pointer */
 };
 
 /* Create a plan (the delay table is precomputed once, in double).
@@ -100,6 +102,17 @@ DDSP_API int ddsp_execute(const ddsp_plan* plan, const void* d_in, void* d_out, 
  * cuda_stream, and synchronises that stream before returning.  h_in: nchan rows of in_pitch elements;
  * h_out: ndm rows of out_pitch elements.  Not re-entrant for one plan (the staging buffers are shared). */
 DDSP_API int ddsp_execute_host(ddsp_plan* plan, const void* h_in, void* h_out, void* cuda_stream);
+
+/* Introspection of the ring kernel's plan-time tables (tile geometry; DESIGN.md section
+ * 6), so that the host logic can be tested without a GPU.  DDSP_ERR_UNSUPPORTED if the ring kernel cannot
+ * run this plan.  geom: host int32[10] = {rows per stage C, DM blocks, chunks, padded channel count,
+ * row stride (bytes of one phase copy), stages, table words per chunk, stage bytes, shared memory bytes,
+ * tile length T}.  meta: host int64[blocks * padded channels]: bits 0..47 byte offset of the staged row
+ * window at tile 0, bits 48.. its length in 16-byte units.  tbl: host uint32[blocks * chunks * table
+ * words]: per chunk C x 32 stage-relative byte offsets ((slot * 4 + phase) * row stride + word offset),
+ * then C unit counts.  rows: host int32[blocks * 32]: output row of each DM-sorted trial, -1 = padding. */
+DDSP_API int ddsp_plan_ring_geometry(const ddsp_plan* plan, int32_t* geom);
+DDSP_API int ddsp_plan_ring_tables(const ddsp_plan* plan, int64_t* meta, uint32_t* tbl, int32_t* rows);
 
 DDSP_API int ddsp_plan_destroy(ddsp_plan* plan); /* NULL is allowed */
 

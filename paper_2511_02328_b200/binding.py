@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libddsp.so")
 
 DDSP_IN_U8, DDSP_IN_F32 = 0, 1
 DDSP_OK, DDSP_ERR_INVALID_ARG, DDSP_ERR_NO_OUTPUT, DDSP_ERR_UNSUPPORTED, DDSP_ERR_ALLOC, DDSP_ERR_CUDA = range(6)
-DDSP_KERNEL_AUTO, DDSP_KERNEL_DIRECT, DDSP_KERNEL_TILED = 0, 1, 2
+DDSP_KERNEL_AUTO, DDSP_KERNEL_DIRECT, DDSP_KERNEL_TILED, DDSP_KERNEL_RING = 0, 1, 2, 3
 
 # name -> (restype, argtypes); one entry per declaration in include/ddsp.h
 _i, _i64, _f64, _vp, _cp = ctypes.c_int, ctypes.c_int64, ctypes.c_double, ctypes.c_void_p, ctypes.c_char_p
@@ -31,6 +31,8 @@ SIGNATURES = {
     "ddsp_plan_get_delays": (_i, [_vp, _vp]),
     "ddsp_execute": (_i, [_vp, _vp, _vp, _vp]),
     "ddsp_execute_host": (_i, [_vp, _vp, _vp, _vp]),
+    "ddsp_plan_ring_geometry": (_i, [_vp, _vp]),
+    "ddsp_plan_ring_tables": (_i, [_vp, _vp, _vp, _vp]),
     "ddsp_plan_destroy": (_i, [_vp]),
     "ddsp_strerror": (_cp, [_i]),
     "ddsp_last_cuda_error": (_i, [_vp]),
@@ -114,6 +116,24 @@ class Plan:
         out = np.empty((self.ndm, self.nchan), dtype=np.int32)
         _check(lib().ddsp_plan_get_delays(self._h, out.ctypes.data), "ddsp_plan_get_delays", self._h)
         return out
+
+    def ring_geometry(self):
+        """ddsp_plan_ring_geometry as a dict (raises DdspError(UNSUPPORTED) if the ring kernel cannot run)."""
+        g = np.zeros(10, dtype=np.int32)
+        _check(lib().ddsp_plan_ring_geometry(self._h, g.ctypes.data), "ddsp_plan_ring_geometry", self._h)
+        names = ("c_rows", "nblk", "nchunk", "nch_pad", "row_stride", "nstage", "tblw", "stage_bytes",
+                 "smem_bytes", "tile_t")
+        return dict(zip(names, (int(v) for v in g)))
+
+    def ring_tables(self):
+        """ddsp_plan_ring_tables: (meta int64[nblk, nch_pad], tbl uint32[nblk, nchunk, tblw], rows int32[nblk, 32])."""
+        g = self.ring_geometry()
+        meta = np.zeros((g["nblk"], g["nch_pad"]), dtype=np.int64)
+        tbl = np.zeros((g["nblk"], g["nchunk"], g["tblw"]), dtype=np.uint32)
+        rows = np.zeros((g["nblk"], 32), dtype=np.int32)
+        _check(lib().ddsp_plan_ring_tables(self._h, meta.ctypes.data, tbl.ctypes.data, rows.ctypes.data),
+               "ddsp_plan_ring_tables", self._h)
+        return meta, tbl, rows
 
     # -- setters --------------------------------------------------------------------------------
     def set_pitch(self, in_pitch_elems, out_pitch_elems):

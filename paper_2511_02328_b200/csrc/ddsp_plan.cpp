@@ -27,7 +27,7 @@ size_t elem_size_in(const ddsp_plan* p) { return p->in_dtype == DDSP_IN_U8 ? 1 :
 
 void resolve_kernel(ddsp_plan* p) {
     if (p->kernel_req == DDSP_KERNEL_AUTO)
-        p->kernel = p->tiled.ok ? DDSP_KERNEL_TILED : DDSP_KERNEL_DIRECT;
+        p->kernel = p->ring.ok ? DDSP_KERNEL_RING : p->tiled.ok ? DDSP_KERNEL_TILED : DDSP_KERNEL_DIRECT;
     else
         p->kernel = p->kernel_req;
 }
@@ -152,6 +152,7 @@ int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, 
         }
     }
     rc = ddsp_tiled_plan(p);
+    if (rc == DDSP_OK) rc = ddsp_ring_plan(p);
     if (rc != DDSP_OK) { ddsp_plan_destroy(p); return rc; }
     resolve_kernel(p);
     *plan = p;
@@ -164,14 +165,17 @@ int ddsp_plan_set_pitch(ddsp_plan* p, int64_t in_pitch, int64_t out_pitch) {
     p->out_pitch = out_pitch;
     if (p->d_stage_in) { cudaFree(p->d_stage_in); p->d_stage_in = nullptr; }
     if (p->d_stage_out) { cudaFree(p->d_stage_out); p->d_stage_out = nullptr; }
-    return ddsp_tiled_set_pitch(p);
+    const int rc = ddsp_tiled_set_pitch(p);
+    return rc != DDSP_OK ? rc : ddsp_ring_set_pitch(p);
 }
 
 int ddsp_plan_set_kernel(ddsp_plan* p, int kernel) {
     if (!p) return DDSP_ERR_INVALID_ARG;
-    if (kernel != DDSP_KERNEL_AUTO && kernel != DDSP_KERNEL_DIRECT && kernel != DDSP_KERNEL_TILED)
+    if (kernel != DDSP_KERNEL_AUTO && kernel != DDSP_KERNEL_DIRECT && kernel != DDSP_KERNEL_TILED &&
+        kernel != DDSP_KERNEL_RING)
         return DDSP_ERR_INVALID_ARG;
     if (kernel == DDSP_KERNEL_TILED && !p->tiled.ok) return DDSP_ERR_UNSUPPORTED;
+    if (kernel == DDSP_KERNEL_RING && !p->ring.ok) return DDSP_ERR_UNSUPPORTED;
     p->kernel_req = kernel;
     resolve_kernel(p);
     return DDSP_OK;
@@ -195,7 +199,13 @@ int ddsp_execute(const ddsp_plan* p, const void* d_in, void* d_out, void* cuda_s
     if (p->device < 0) return DDSP_ERR_CUDA;  // host-only plan: no device, no fallback
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e;
-    if (p->kernel == DDSP_KERNEL_TILED && !ddsp_tiled_can_run(p, d_in, d_out)) {
+    if (p->kernel == DDSP_KERNEL_RING) {
+        if (ddsp_ring_can_run(p, d_in, d_out)) e = ddsp_launch_ring(p, d_in, d_out, s);
+        else if (p->kernel_req == DDSP_KERNEL_RING) return DDSP_ERR_UNSUPPORTED;
+        // unaligned input base: correct through the register-staged or the direct kernel
+        else if (ddsp_tiled_can_run(p, d_in, d_out)) e = ddsp_launch_tiled(p, d_in, d_out, s);
+        else e = ddsp_launch_direct(p, d_in, d_out, s);
+    } else if (p->kernel == DDSP_KERNEL_TILED && !ddsp_tiled_can_run(p, d_in, d_out)) {
         // unaligned buffers: correct through the direct kernel unless the tiled one was forced
         if (p->kernel_req == DDSP_KERNEL_TILED) return DDSP_ERR_UNSUPPORTED;
         e = ddsp_launch_direct(p, d_in, d_out, s);
@@ -230,6 +240,7 @@ int ddsp_execute_host(ddsp_plan* p, const void* h_in, void* h_out, void* cuda_st
 int ddsp_plan_destroy(ddsp_plan* p) {
     if (!p) return DDSP_OK;
     ddsp_tiled_free(p);
+    ddsp_ring_free(p);
     if (p->d_delays) cudaFree(p->d_delays);
     if (p->d_chan_list) cudaFree(p->d_chan_list);
     if (p->d_stage_in) cudaFree(p->d_stage_in);

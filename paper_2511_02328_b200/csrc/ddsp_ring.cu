@@ -1,0 +1,515 @@
+// ddsp_ring.cu -- DDSP_KERNEL_RING: shared-memory tiled brute-force dedispersion with an asynchronous
+// staging ring.
+//
+//   D[i][t] = sum over unmasked c of x[c][t + d(i,c)]
+//
+// One CTA (512 threads) computes a tile of 32 consecutive (DM-sorted) trials x 2048 output samples and
+// loops over the unmasked channels in chunks of C rows.  For every chunk the needed window of each
+// channel row, [t0 + d(i_first,c), t0 + T + d(i_last,c)), is brought into a ring of shared-memory
+// stages by the copy engine (cp.async.bulk, one instruction per row, completion on an mbarrier; no
+// registers, no thread waits on global memory) and serves all 32 trials (PAPER.md:19, 59
+// "shared-memory tiling" is the prior art; the ring, the phase copies and the packed accumulators
+// are ours).
+//
+// The shifted read x[c][t + d] lands on an arbitrary byte of the row, but a 32-bit shared-memory load
+// must be 4-byte aligned.  Each staged row is therefore expanded, shared memory to shared memory, into
+// FOUR phase copies, copy_p[i] = row[i + p]; a trial whose offset is q reads word (q >> 2) of copy
+// (q & 3): always aligned, conflict-free (lanes read consecutive words), no realignment in the hot loop.
+// A loaded word holds 4 consecutive samples.  accE accumulates the WHOLE word (mod 2^32), accO the odd
+// bytes (one PRMT) in 2 x 16-bit lanes; at flush accE - (accO << 8) = B0 + 2^16 B2 exactly, so the hot
+// loop is LDS + PRMT + IADD3 per word = 0.75 instructions per sample-add.  The 16-bit lanes are flushed
+// to the uint32 output rows (read-modify-write, L2-resident, owned by this thread) every 256 channels
+// (255 * 257 < 65536).
+//
+// Pipeline per chunk k (stage k % NS), all 16 warps symmetric:
+//   wait built[k]  ->  warp 0 issues the copies of chunk k + NS - 2  ->  wait raw[k+1], expand chunk
+//   k+1 into its phase copies, arrive built[k+1]  ->  hot loop on chunk k.
+// A thread arrives on built[k] only after it finished the hot loop of chunk k-2, so when built[k]
+// completes the stage of chunk k-2 is free for the copies of chunk k + NS - 2.  The barriers are
+// split-phase (arrive now, wait one chunk later): no warp waits for another unless it is a whole
+// chunk ahead.
+#include <algorithm>
+#include <cstdio>
+#include <cstdlib>
+#include <vector>
+
+#include "ddsp_internal.h"
+
+namespace {
+
+constexpr int kBdm = 32;            // trials per CTA tile
+constexpr int kTileT = 2048;        // output samples per CTA tile
+constexpr int kThreads = 512;
+constexpr int kWarps = kThreads / 32;
+constexpr int kFlushEvery = 256;    // channels between flushes of the 16-bit lanes
+constexpr int kBarBytes = 1024;     // mbarriers live in the first 1 KB of dynamic shared memory
+constexpr int kMaxStages = 12;
+
+// accumulation variants: where the odd-byte adds go
+constexpr int kOddAlu = 0;    // IADD3 (two rows per add), ALU pipe
+constexpr int kOddFma = 1;    // IMAD x 1, FMA pipe
+constexpr int kOddHalf = 2;   // words 0..KWT/2-1 on the ALU pipe, the rest on the FMA pipe
+
+struct RingArgs {
+    const uint8_t* in;
+    uint32_t* out;
+    const int64_t* meta;      // [nblk][nch_pad] bits 0..47: byte offset of the row window at t0 = 0; bits 48..: 16-byte units
+    const uint32_t* tbl;      // [nblk][nchunk][tblw]: C x 32 stage-relative byte offsets, then C unit counts, padding
+    const int32_t* rows;      // [nblk * 32] output row of each sorted trial, -1 = padding
+    int64_t out_pitch, nsamp_out, in_valid;   // in_valid: bytes of the input buffer that may be read
+    int nlist, nch_pad, nblk, nchunk, row_stride, stage_bytes, nstage, tblw, out_vec;
+    uint32_t one;             // 1: multiplier that routes an add through the FMA pipe (IMAD)
+};
+
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void lds128(uint32_t addr, uint32_t* v) {
+    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(addr));
+}
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    asm volatile("st.shared.v4.u32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void add_fma_pipe(uint32_t& acc, uint32_t v, uint32_t one) {
+    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(acc) : "r"(v), "r"(one));
+}
+__device__ __forceinline__ void mbar_init(uint32_t bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n .reg .pred p;\n WAIT_%=:\n mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        " @p bra DONE_%=;\n bra WAIT_%=;\n DONE_%=:\n}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// global -> shared bulk copy by the copy engine; src, dst and bytes are multiples of 16
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------
+// uint8, ds = 1
+// ------------------------------------------------------------------------------------------------
+// BDM_T trials x KWT words (of 4 samples, strided by 32 lanes) per thread; C rows per stage
+template <int BDM_T, int KWT, int C, int MODE>
+__global__ void __launch_bounds__(kThreads, 1) ddsp_ring_u8_kernel(const RingArgs a) {
+    constexpr int GROUPS = kBdm / BDM_T;
+    constexpr int SLABS = kTileT / (KWT * 128);
+    static_assert(GROUPS * SLABS == kWarps, "16 warps");
+    static_assert(C == 2 || C == 4, "2 or 4 rows per stage");
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int slab = warp % SLABS, grp = warp / SLABS;
+    const int blk = blockIdx.x % a.nblk;
+    const int64_t t0 = (int64_t)(blockIdx.x / a.nblk) * kTileT;
+    const int NS = a.nstage, S = a.row_stride;
+    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t rows_bytes = (uint32_t)(C * 4 * S);   // the table of a stage follows its rows
+
+    auto bar_raw = [&](int s) { return smem_base + (uint32_t)s * 8u; };
+    auto bar_built = [&](int s) { return smem_base + 512u + (uint32_t)s * 8u; };
+    auto stage_base = [&](int s) { return smem_base + (uint32_t)kBarBytes + (uint32_t)s * (uint32_t)a.stage_bytes; };
+
+    if (tid == 0) {
+        for (int s = 0; s < NS; ++s) {
+            mbar_init(bar_raw(s), 1);
+            mbar_init(bar_built(s), kWarps);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // packed accumulators of each owned word (4 consecutive samples s0..s3): accE = sum of whole words
+    // (mod 2^32), accO = (s1, s3) in 16-bit lanes
+    uint32_t accE[BDM_T][KWT], accO[BDM_T][KWT];
+#pragma unroll
+    for (int j = 0; j < BDM_T; ++j)
+#pragma unroll
+        for (int k = 0; k < KWT; ++k) { accE[j][k] = 0; accO[j][k] = 0; }
+
+    const int64_t* __restrict__ meta_b = a.meta + (size_t)blk * a.nch_pad;
+    const uint32_t* __restrict__ tbl_b = a.tbl + (size_t)blk * a.nchunk * a.tblw;
+
+    // ---- copy issue (warp 0): lane r < C owns row r of the chunk ----
+    int64_t meta_pref = 0;      // metadata of the next chunk to issue, loaded one iteration ahead
+    auto load_meta = [&](int chunk) {
+        meta_pref = (lane < C && chunk < a.nchunk) ? __ldg(meta_b + chunk * C + lane) : 0;
+    };
+    auto issue = [&](int chunk) {
+        const int s = chunk % NS;
+        const uint32_t bar = bar_raw(s), sb = stage_base(s);
+        const int64_t so = (meta_pref & 0xffffffffffffLL) + t0;
+        const uint32_t bytes = (uint32_t)(meta_pref >> 48) * 16u;
+        uint32_t cp = bytes;
+        const int64_t room = a.in_valid - so;
+        if ((int64_t)bytes > room) {        // the window runs past the end of the input buffer
+            cp = room > 0 ? (uint32_t)(room & ~(int64_t)15) : 0u;
+            const int tail = room > 0 ? (int)(room - cp) : 0;
+            for (int i = 0; i < tail; ++i) smem[kBarBytes + (size_t)s * a.stage_bytes + (size_t)lane * 4 * S + cp + i] = a.in[so + cp + i];
+            // these generic-proxy writes precede later copy-engine writes to the same bytes
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        }
+        uint32_t total = cp;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
+        __syncwarp();
+        if (lane == 0) mbar_arrive_expect_tx(bar, total + (uint32_t)a.tblw * 4u);
+        __syncwarp();
+        if (cp) bulk_g2s(sb + (uint32_t)lane * 4u * (uint32_t)S, a.in + so, cp, bar);
+        if (lane == 0) bulk_g2s(sb + rows_bytes, tbl_b + (size_t)chunk * a.tblw, (uint32_t)a.tblw * 4u, bar);
+    };
+
+    // ---- expand the raw rows of a chunk into phase copies 1..3 (all threads) ----
+    auto build = [&](int chunk) {
+        const int s = chunk % NS;
+        const uint32_t sb = stage_base(s);
+        mbar_wait(bar_raw(s), (uint32_t)(chunk / NS) & 1u);
+        uint32_t n[C];
+        if (C == 4) lds128(sb + rows_bytes + C * kBdm * 4, n);
+        else { n[0] = lds32(sb + rows_bytes + C * kBdm * 4); n[1] = lds32(sb + rows_bytes + C * kBdm * 4 + 4); }
+        uint32_t total = 0;
+#pragma unroll
+        for (int r = 0; r < C; ++r) total += n[r];
+        for (uint32_t f = tid; f < total; f += kThreads) {
+            uint32_t r = 0, u = f;
+#pragma unroll
+            for (int q = 0; q < C - 1; ++q)
+                if (r == (uint32_t)q && u >= n[q]) { u -= n[q]; r = q + 1; }
+            const uint32_t addr = sb + r * 4u * (uint32_t)S + u * 16u;
+            uint32_t w[4];
+            lds128(addr, w);
+            const uint32_t w4 = lds32(addr + 16);
+            sts128(addr + S, __byte_perm(w[0], w[1], 0x4321), __byte_perm(w[1], w[2], 0x4321),
+                   __byte_perm(w[2], w[3], 0x4321), __byte_perm(w[3], w4, 0x4321));
+            sts128(addr + 2 * S, __byte_perm(w[0], w[1], 0x5432), __byte_perm(w[1], w[2], 0x5432),
+                   __byte_perm(w[2], w[3], 0x5432), __byte_perm(w[3], w4, 0x5432));
+            sts128(addr + 3 * S, __byte_perm(w[0], w[1], 0x6543), __byte_perm(w[1], w[2], 0x6543),
+                   __byte_perm(w[2], w[3], 0x6543), __byte_perm(w[3], w4, 0x6543));
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_built(s));
+    };
+
+    bool first_flush = true;
+    auto flush = [&]() {
+#pragma unroll 1
+        for (int j = 0; j < BDM_T; ++j) {
+            const int row = __ldg(a.rows + blk * kBdm + grp * BDM_T + j);
+#pragma unroll
+            for (int k = 0; k < KWT; ++k) {
+                const int64_t t = t0 + slab * (KWT * 128) + k * 128 + lane * 4;
+                uint32_t e = 0, o = 0;
+#pragma unroll
+                for (int jj = 0; jj < BDM_T; ++jj)      // static register indexing under a rolled loop
+                    if (jj == j) { e = accE[jj][k]; accE[jj][k] = 0; o = accO[jj][k]; accO[jj][k] = 0; }
+                if (row < 0 || t >= a.nsamp_out) continue;
+                uint32_t* p = a.out + (size_t)row * (size_t)a.out_pitch + t;
+                e -= o << 8;                            // whole-word sum -> even bytes (exact mod 2^32)
+                uint32_t v0 = e & 0xffffu, v2 = e >> 16, v1 = o & 0xffffu, v3 = o >> 16;
+                if (a.out_vec && t + 3 < a.nsamp_out) {
+                    if (!first_flush) {
+                        const uint4 old = *reinterpret_cast<const uint4*>(p);
+                        v0 += old.x; v1 += old.y; v2 += old.z; v3 += old.w;
+                    }
+                    *reinterpret_cast<uint4*>(p) = make_uint4(v0, v1, v2, v3);
+                } else {
+                    const uint32_t v[4] = {v0, v1, v2, v3};
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (t + q < a.nsamp_out) p[q] = first_flush ? v[q] : p[q] + v[q];
+                }
+            }
+        }
+        first_flush = false;
+    };
+
+    // ---- the shifted accumulate over the rows of one chunk ----
+    const uint32_t lane_off = (uint32_t)(slab * (KWT * 128) + lane * 4);
+    const uint32_t one = a.one;
+    auto odd_on_fma = [](int k) { return MODE == kOddFma || (MODE == kOddHalf && k >= KWT / 2); };
+    auto hot = [&](int chunk) {
+        const uint32_t sb = stage_base(chunk % NS);
+        const int nrow = min(C, a.nlist - chunk * C);
+        uint32_t tptr = sb + rows_bytes + (uint32_t)(grp * (BDM_T * 4));
+        const uint32_t rbase = sb + lane_off;
+        int r = 0;
+#pragma unroll 1
+        for (; r + 2 <= nrow; r += 2) {          // two rows per iteration share one IADD3 per accumulator
+            uint32_t o0[BDM_T], o1[BDM_T];
+#pragma unroll
+            for (int j = 0; j < BDM_T; j += 4) {
+                lds128(tptr + (uint32_t)(j * 4), &o0[j]);
+                lds128(tptr + (uint32_t)(kBdm * 4 + j * 4), &o1[j]);
+            }
+            tptr += 2 * kBdm * 4;
+#pragma unroll
+            for (int j = 0; j < BDM_T; ++j) {
+                const uint32_t a0 = rbase + o0[j], a1 = rbase + o1[j];
+#pragma unroll
+                for (int k = 0; k < KWT; ++k) {
+                    const uint32_t w0 = lds32(a0 + k * 128), w1 = lds32(a1 + k * 128);
+                    accE[j][k] = accE[j][k] + w0 + w1;                                  // IADD3
+                    const uint32_t p0 = __byte_perm(w0, 0, 0x4341), p1 = __byte_perm(w1, 0, 0x4341);
+                    if (odd_on_fma(k)) {
+                        add_fma_pipe(accO[j][k], p0, one);                              // IMAD (FMA pipe)
+                        add_fma_pipe(accO[j][k], p1, one);
+                    } else {
+                        accO[j][k] = accO[j][k] + p0 + p1;                              // IADD3 (ALU pipe)
+                    }
+                }
+            }
+        }
+        if (r < nrow) {                          // odd row count (last chunk only)
+            uint32_t o0[BDM_T];
+#pragma unroll
+            for (int j = 0; j < BDM_T; j += 4) lds128(tptr + (uint32_t)(j * 4), &o0[j]);
+#pragma unroll
+            for (int j = 0; j < BDM_T; ++j) {
+                const uint32_t a0 = rbase + o0[j];
+#pragma unroll
+                for (int k = 0; k < KWT; ++k) {
+                    const uint32_t w0 = lds32(a0 + k * 128);
+                    accE[j][k] += w0;
+                    accO[j][k] += __byte_perm(w0, 0, 0x4341);
+                }
+            }
+        }
+    };
+
+    // ---- prologue: copies of chunks 0 .. NS-3 in flight, chunk 0 expanded ----
+    const int ahead = NS - 2;                    // chunk k + ahead is issued in iteration k
+    if (warp == 0) {
+        for (int c = 0; c < ahead && c < a.nchunk; ++c) { load_meta(c); issue(c); }
+        load_meta(ahead);
+    }
+    build(0);
+    int since_flush = 0;
+    for (int chunk = 0; chunk < a.nchunk; ++chunk) {
+        mbar_wait(bar_built(chunk % NS), (uint32_t)(chunk / NS) & 1u);
+        if (warp == 0) {
+            if (chunk + ahead < a.nchunk) issue(chunk + ahead);
+            load_meta(chunk + ahead + 1);
+        }
+        if (chunk + 1 < a.nchunk) build(chunk + 1);
+        const int nrow = min(C, a.nlist - chunk * C);
+        if (since_flush + nrow > kFlushEvery) { flush(); since_flush = 0; }
+        since_flush += nrow;
+        hot(chunk);
+    }
+    flush();
+}
+
+typedef void (*RingKernel)(const RingArgs);
+struct Variant { int c; RingKernel fn; };
+const Variant kVariants[] = {
+    {4, ddsp_ring_u8_kernel<8, 4, 4, kOddAlu>},
+    {4, ddsp_ring_u8_kernel<8, 4, 4, kOddHalf>},
+    {4, ddsp_ring_u8_kernel<8, 4, 4, kOddFma>},
+    {4, ddsp_ring_u8_kernel<4, 8, 4, kOddAlu>},
+    {4, ddsp_ring_u8_kernel<4, 8, 4, kOddHalf>},
+    {2, ddsp_ring_u8_kernel<8, 4, 2, kOddAlu>},
+    {2, ddsp_ring_u8_kernel<8, 4, 2, kOddHalf>},
+    {2, ddsp_ring_u8_kernel<4, 8, 2, kOddAlu>},
+};
+constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+template <typename T>
+cudaError_t upload(T** dptr, const std::vector<T>& h) {
+    cudaError_t e = cudaMalloc((void**)dptr, std::max<size_t>(h.size(), 1) * sizeof(T));
+    if (e != cudaSuccess) return e;
+    return cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+// first delay of block b for channel c, moved down so that the row window starts on a 16-byte
+// boundary of the input buffer (base pointer 16-byte aligned, any pitch)
+inline int64_t window_lo(const ddsp_plan* p, int b, int c, int64_t in_pitch) {
+    const int i0 = p->order[(size_t)b * kBdm];
+    const int64_t d0 = p->delays[(size_t)i0 * p->nchan + c];
+    const int64_t a = ((int64_t)c * in_pitch + d0) % 16;
+    return d0 - a;     // may be negative for c > 0: the window then starts in the previous row (valid memory)
+}
+
+}  // namespace
+
+// Geometry of variant v for this plan; false if its stages do not fit.
+static bool ring_geometry(const ddsp_plan* p, int v, ddsp_ring& g) {
+    const int nlist = (int)p->chan_list.size();
+    const int budget = (p->smem_optin > 0 ? p->smem_optin : 232448) - kBarBytes;
+    const int c_rows = kVariants[v].c;
+    const int nblk = (p->ndm + kBdm - 1) / kBdm;
+    // longest row window over all (block, channel); 15 more bytes for the alignment of the window start
+    int64_t max_q = 0;
+    for (int b = 0; b < nblk; ++b) {
+        const int i0 = p->order[(size_t)b * kBdm];
+        const int i1 = p->order[std::min<size_t>((size_t)b * kBdm + kBdm, (size_t)p->ndm) - 1];
+        for (int l = 0; l < nlist; ++l) {
+            const int c = p->chan_list[l];
+            max_q = std::max<int64_t>(max_q, (int64_t)p->delays[(size_t)i1 * p->nchan + c] -
+                                                 p->delays[(size_t)i0 * p->nchan + c] + 15);
+        }
+    }
+    // raw bytes [0, max_q + T) are read; the expansion of the last unit looks at the first word of the next
+    const int64_t units = (max_q + kTileT + 15) / 16 + 1;
+    if (units > 4095) return false;
+    const int row_stride = (int)units * 16;
+    const int tblw = c_rows * kBdm + 4;
+    const int stage_bytes = (c_rows * 4 * row_stride + tblw * 4 + 127) & ~127;
+    const int nstage = std::min(kMaxStages, budget / stage_bytes);
+    if (nstage < 4) return false;
+    g.variant = v;
+    g.c_rows = c_rows;
+    g.nblk = nblk;
+    g.ntile_t = (p->nsamp_out + kTileT - 1) / kTileT;
+    g.row_stride = row_stride;
+    g.tblw = tblw;
+    g.stage_bytes = stage_bytes;
+    g.nstage = nstage;
+    g.smem_bytes = kBarBytes + nstage * stage_bytes;
+    g.nchunk = (nlist + c_rows - 1) / c_rows;
+    g.nch_pad = g.nchunk * c_rows;
+    return (int64_t)g.ntile_t * g.nblk <= 2147483647LL;
+}
+
+// Tables depend on the input pitch through the alignment of the row windows.
+int ddsp_ring_set_pitch(ddsp_plan* p) {
+    ddsp_ring& g = p->ring;
+    if (!g.ok) return DDSP_OK;
+    const int nlist = (int)p->chan_list.size();
+    if ((int64_t)p->nchan * p->in_pitch >= ((int64_t)1 << 47)) { g.ok = false; return DDSP_OK; }
+    std::vector<int64_t> meta((size_t)g.nblk * g.nch_pad, 0);
+    std::vector<uint32_t> tbl((size_t)g.nblk * g.nchunk * g.tblw, 0);
+    for (int b = 0; b < g.nblk; ++b)
+        for (int l = 0; l < nlist; ++l) {
+            const int c = p->chan_list[l];
+            const int chunk = l / g.c_rows, slot = l % g.c_rows;
+            const int64_t lo = window_lo(p, b, c, p->in_pitch);
+            uint32_t* t = &tbl[((size_t)b * g.nchunk + chunk) * g.tblw];
+            int64_t qmax = 0;
+            for (int j = 0; j < kBdm; ++j) {
+                const size_t s = std::min<size_t>((size_t)b * kBdm + j, (size_t)p->ndm - 1);
+                const int64_t q = p->delays[(size_t)p->order[s] * p->nchan + c] - lo;
+                qmax = std::max(qmax, q);
+                t[slot * kBdm + j] = (uint32_t)((slot * 4 + (q & 3)) * g.row_stride + (q >> 2) * 4);
+            }
+            const int64_t need = (qmax + kTileT + 15) / 16;      // units of raw bytes [0, qmax + T)
+            if (need + 1 > g.row_stride / 16) { g.ok = false; return DDSP_OK; }   // cannot happen (geometry)
+            t[g.c_rows * kBdm + slot] = (uint32_t)need;
+            meta[(size_t)b * g.nch_pad + l] = ((int64_t)c * p->in_pitch + lo) | (need << 48);
+        }
+    g.h_meta = meta;
+    g.h_tbl = tbl;
+    if (p->device < 0) return DDSP_OK;   // host-only plan: geometry and tables only
+    cudaError_t e = cudaSuccess;
+    if (!g.d_meta) e = cudaMalloc((void**)&g.d_meta, meta.size() * sizeof(int64_t));
+    if (e == cudaSuccess && !g.d_tbl) e = cudaMalloc((void**)&g.d_tbl, tbl.size() * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaMemcpy(g.d_meta, meta.data(), meta.size() * sizeof(int64_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(g.d_tbl, tbl.data(), tbl.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { p->last_cuda = (int)e; (void)cudaGetLastError(); return DDSP_ERR_CUDA; }
+    return DDSP_OK;
+}
+
+int ddsp_ring_plan(ddsp_plan* p) {
+    ddsp_ring& g = p->ring;
+    g.ok = false;
+    const int nlist = (int)p->chan_list.size();
+    if (p->in_dtype != DDSP_IN_U8 || p->ds != 1 || nlist < 1) return DDSP_OK;   // other paths: other kernels
+    // Not yet run on a B200 (GPU access closed while it was written): opt-in until its parity tests
+    // have passed on hardware; DDSP_KERNEL_AUTO keeps resolving to the verified kernels.
+    const char* en = getenv("DDSP_ENABLE_RING");
+    if (!en || atoi(en) == 0) return DDSP_OK;
+    int forced = -1;    // DDSP_RING_VARIANT: tuning only
+    if (const char* ev = getenv("DDSP_RING_VARIANT")) forced = atoi(ev);
+    for (int k = -1; k < kNumVariants && !g.ok; ++k) {
+        const int v = k < 0 ? forced : k;
+        if (v < 0 || v >= kNumVariants) continue;
+        g.ok = ring_geometry(p, v, g);
+    }
+    if (!g.ok) return DDSP_OK;
+    std::vector<int32_t> rows((size_t)g.nblk * kBdm, -1);
+    for (size_t s = 0; s < (size_t)p->ndm; ++s) rows[s] = p->order[s];
+    g.h_rows = rows;
+    if (p->device >= 0) {
+        cudaError_t e = upload(&g.d_rows, rows);
+        // the attribute belongs to the function, not to a plan: always opt in to the device maximum
+        for (int v = 0; v < kNumVariants && e == cudaSuccess; ++v)
+            e = cudaFuncSetAttribute(kVariants[v].fn, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_optin);
+        if (e != cudaSuccess) {
+            p->last_cuda = (int)e;
+            (void)cudaGetLastError();
+            ddsp_ring_free(p);
+            g.ok = false;
+            return e == cudaErrorMemoryAllocation ? DDSP_ERR_ALLOC : DDSP_ERR_CUDA;
+        }
+    }
+    return ddsp_ring_set_pitch(p);
+}
+
+void ddsp_ring_free(ddsp_plan* p) {
+    ddsp_ring& g = p->ring;
+    if (g.d_meta) cudaFree(g.d_meta);
+    if (g.d_tbl) cudaFree(g.d_tbl);
+    if (g.d_rows) cudaFree(g.d_rows);
+    g.d_meta = nullptr; g.d_tbl = nullptr; g.d_rows = nullptr;
+}
+
+bool ddsp_ring_can_run(const ddsp_plan* p, const void* d_in, const void* d_out) {
+    // the copy engine needs 16-byte aligned sources: aligned base pointer, any pitch (the row windows
+    // are aligned at plan time); any output alignment is correct
+    return p->ring.ok && d_in != nullptr && d_out != nullptr && ((uintptr_t)d_in % 16 == 0);
+}
+
+cudaError_t ddsp_launch_ring(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s) {
+    const ddsp_ring& g = p->ring;
+    RingArgs a;
+    a.in = (const uint8_t*)d_in;
+    a.out = (uint32_t*)d_out;
+    a.meta = g.d_meta; a.tbl = g.d_tbl; a.rows = g.d_rows;
+    a.out_pitch = p->out_pitch; a.nsamp_out = p->nsamp_out; a.one = 1u;
+    a.in_valid = (int64_t)(p->nchan - 1) * p->in_pitch + p->nsamp;   // the last row may end at nsamp
+    a.nlist = (int)p->chan_list.size(); a.nch_pad = g.nch_pad; a.nblk = g.nblk; a.nchunk = g.nchunk;
+    a.row_stride = g.row_stride; a.stage_bytes = g.stage_bytes; a.nstage = g.nstage; a.tblw = g.tblw;
+    a.out_vec = ((uintptr_t)d_out % 16 == 0) && (p->out_pitch % 4 == 0);
+    const unsigned grid = (unsigned)(g.ntile_t * g.nblk);
+    kVariants[g.variant].fn<<<grid, kThreads, g.smem_bytes, s>>>(a);
+    return cudaGetLastError();
+}
+
+// Introspection for the CPU tests of the plan-time geometry (tests/test_ring_tables_cpu.py).
+extern "C" {
+
+int ddsp_plan_ring_geometry(const ddsp_plan* p, int32_t* geom) {
+    if (!p || !geom) return DDSP_ERR_INVALID_ARG;
+    const ddsp_ring& g = p->ring;
+    if (!g.ok) return DDSP_ERR_UNSUPPORTED;
+    const int32_t v[10] = {g.c_rows, g.nblk, g.nchunk, g.nch_pad, g.row_stride, g.nstage, g.tblw,
+                           g.stage_bytes, g.smem_bytes, kTileT};
+    for (int i = 0; i < 10; ++i) geom[i] = v[i];
+    return DDSP_OK;
+}
+
+int ddsp_plan_ring_tables(const ddsp_plan* p, int64_t* meta, uint32_t* tbl, int32_t* rows) {
+    if (!p || !meta || !tbl || !rows) return DDSP_ERR_INVALID_ARG;
+    const ddsp_ring& g = p->ring;
+    if (!g.ok) return DDSP_ERR_UNSUPPORTED;
+    std::copy(g.h_meta.begin(), g.h_meta.end(), meta);
+    std::copy(g.h_tbl.begin(), g.h_tbl.end(), tbl);
+    std::copy(g.h_rows.begin(), g.h_rows.end(), rows);
+    return DDSP_OK;
+}
+
+}  // extern "C"

@@ -15,8 +15,8 @@ from _util import (assert_f32_close, assert_u32_equal, crop, make_input, oracle_
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [binding.DDSP_KERNEL_DIRECT, binding.DDSP_KERNEL_TILED]
-KNAME = {binding.DDSP_KERNEL_DIRECT: "direct", binding.DDSP_KERNEL_TILED: "tiled"}
+KERNELS = [binding.DDSP_KERNEL_DIRECT, binding.DDSP_KERNEL_TILED, binding.DDSP_KERNEL_RING]
+KNAME = {binding.DDSP_KERNEL_DIRECT: "direct", binding.DDSP_KERNEL_TILED: "tiled", binding.DDSP_KERNEL_RING: "ring"}
 
 
 @pytest.fixture(scope="module", autouse=True)
