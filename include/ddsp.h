@@ -59,7 +59,8 @@ enum {
     DDSP_KERNEL_DIRECT = 1, /* one thread per output element, reads global memory directly (any plan) */
     DDSP_KERNEL_TILED = 2,  /* shared-memory tiled kernel, rows staged through registers (first version) */
     DDSP_KERNEL_RING = 3    /* shared-memory tiled kernel, rows staged by the copy engine into an mbarrier ring
-                               (DESIGN.md section 6); needs a 16-byte aligned input base pointer */
+                               (DESIGN.md section 6); needs a 16-byte aligned input base pointer; uint8 with ds > 1 also
+                               a row pitch that is a multiple of 16; float32 only with ds = 1 */
 };
 
 /* Create a plan (the delay table is precomputed once, in double).
@@ -113,6 +114,15 @@ DDSP_API int ddsp_execute_host(ddsp_plan* plan, const void* h_in, void* h_out, v
  * then C unit counts.  rows: host int32[blocks * 32]: output row of each DM-sorted trial, -1 = padding. */
 DDSP_API int ddsp_plan_ring_geometry(const ddsp_plan* plan, int32_t* geom);
 DDSP_API int ddsp_plan_ring_tables(const ddsp_plan* plan, int64_t* meta, uint32_t* tbl, int32_t* rows);
+/* The same for the ring kernels of float32 input (ds = 1) and of uint8 input with ds > 1 (ddsp_ringx.cu).
+ * geom: host int32[14] = {kind (1: uint8 16-bit bins, 2: float32), rows per chunk C, DM blocks, chunks,
+ * padded channel count, raw row stride (bytes), bins row stride (bytes of one phase copy; kind 1), table words
+ * per chunk, raw slots, bin slots, shared memory bytes, tile length T, channels between flushes (kind 1), raw
+ * slot bytes}.  meta as above (byte offsets).  tbl per chunk: C x 32 byte offsets (kind 2: slot * raw stride +
+ * 4 q; kind 1: (slot * 2 + (q & 1)) * bins stride + (q >> 1) * 4), then C unit counts (kind 2: 16-byte units of
+ * the window; kind 1: 8-bin units), then (kind 1) C raw byte indices of the window start within the row. */
+DDSP_API int ddsp_plan_ringx_geometry(const ddsp_plan* plan, int32_t* geom);
+DDSP_API int ddsp_plan_ringx_tables(const ddsp_plan* plan, int64_t* meta, uint32_t* tbl, int32_t* rows);
 
 DDSP_API int ddsp_plan_destroy(ddsp_plan* plan); /* NULL is allowed */
 

@@ -33,6 +33,8 @@ SIGNATURES = {
     "ddsp_execute_host": (_i, [_vp, _vp, _vp, _vp]),
     "ddsp_plan_ring_geometry": (_i, [_vp, _vp]),
     "ddsp_plan_ring_tables": (_i, [_vp, _vp, _vp, _vp]),
+    "ddsp_plan_ringx_geometry": (_i, [_vp, _vp]),
+    "ddsp_plan_ringx_tables": (_i, [_vp, _vp, _vp, _vp]),
     "ddsp_plan_destroy": (_i, [_vp]),
     "ddsp_strerror": (_cp, [_i]),
     "ddsp_last_cuda_error": (_i, [_vp]),
@@ -133,6 +135,22 @@ class Plan:
         rows = np.zeros((g["nblk"], 32), dtype=np.int32)
         _check(lib().ddsp_plan_ring_tables(self._h, meta.ctypes.data, tbl.ctypes.data, rows.ctypes.data),
                "ddsp_plan_ring_tables", self._h)
+        return meta, tbl, rows
+
+    def ringx_geometry(self):
+        g = np.zeros(14, dtype=np.int32)
+        _check(lib().ddsp_plan_ringx_geometry(self._h, g.ctypes.data), "ddsp_plan_ringx_geometry", self._h)
+        names = ("kind", "c_rows", "nblk", "nchunk", "nch_pad", "raw_stride", "bins_stride", "tblw", "nraw",
+                 "nbins", "smem_bytes", "tile_t", "flush_every", "raw_slot_bytes")
+        return dict(zip(names, (int(v) for v in g)))
+
+    def ringx_tables(self):
+        g = self.ringx_geometry()
+        meta = np.zeros((g["nblk"], g["nch_pad"]), dtype=np.int64)
+        tbl = np.zeros((g["nblk"], g["nchunk"], g["tblw"]), dtype=np.uint32)
+        rows = np.zeros((g["nblk"], 32), dtype=np.int32)
+        _check(lib().ddsp_plan_ringx_tables(self._h, meta.ctypes.data, tbl.ctypes.data, rows.ctypes.data),
+               "ddsp_plan_ringx_tables", self._h)
         return meta, tbl, rows
 
     # -- setters --------------------------------------------------------------------------------

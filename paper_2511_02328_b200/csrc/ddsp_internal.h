@@ -56,6 +56,29 @@ struct ddsp_ring {
     std::vector<int32_t> h_rows;
 };
 
+// Geometry of the ring kernels for float32 input and for uint8 input with ds > 1 (ddsp_ringx.cu).
+struct ddsp_ringx {
+    bool ok = false;
+    int kind = 0;          // 1: uint8, ds > 1 (16-bit bins); 2: float32, ds = 1
+    int variant = 0;
+    int c_rows = 0;        // channel rows per chunk
+    int nblk = 0;          // DM blocks of 32 sorted trials
+    int tile_t = 0;        // output samples per tile
+    int64_t ntile_t = 0;
+    int raw_stride = 0;    // bytes per staged raw row
+    int bins_stride = 0;   // kind 1: bytes per phase copy of the 16-bit bins of a row
+    int tblw = 0;          // 32-bit words of the per-chunk table
+    int raw_slot_bytes = 0, bins_slot_bytes = 0, nraw = 0, nbins = 0, smem_bytes = 0;
+    int nchunk = 0, nch_pad = 0;
+    int flush_every = 0;   // kind 1: channels between flushes of the 16-bit lanes
+    int64_t* d_meta = nullptr;
+    uint32_t* d_tbl = nullptr;
+    int32_t* d_rows = nullptr;
+    std::vector<int64_t> h_meta;
+    std::vector<uint32_t> h_tbl;
+    std::vector<int32_t> h_rows;
+};
+
 struct ddsp_plan {
     // problem
     int nchan = 0, ndm = 0, ds = 1, in_dtype = DDSP_IN_U8;
@@ -75,6 +98,7 @@ struct ddsp_plan {
     int32_t* d_chan_list = nullptr;  // [nchan_unmasked]
     ddsp_tiled tiled;
     ddsp_ring ring;
+    ddsp_ringx ringx;
     int kernel_req = DDSP_KERNEL_AUTO;
     int kernel = DDSP_KERNEL_DIRECT;
     mutable int last_cuda = 0;
@@ -101,3 +125,10 @@ int ddsp_ring_set_pitch(ddsp_plan* p);    // rebuilds the pitch-dependent tables
 void ddsp_ring_free(ddsp_plan* p);
 bool ddsp_ring_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);   // 16-byte aligned input base
 cudaError_t ddsp_launch_ring(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);
+
+// ddsp_ringx.cu (same entry points as the ring kernel, for float32 and for uint8 with ds > 1)
+int ddsp_ringx_plan(ddsp_plan* p);
+int ddsp_ringx_set_pitch(ddsp_plan* p);
+void ddsp_ringx_free(ddsp_plan* p);
+bool ddsp_ringx_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);
+cudaError_t ddsp_launch_ringx(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);

@@ -27,7 +27,7 @@ size_t elem_size_in(const ddsp_plan* p) { return p->in_dtype == DDSP_IN_U8 ? 1 :
 
 void resolve_kernel(ddsp_plan* p) {
     if (p->kernel_req == DDSP_KERNEL_AUTO)
-        p->kernel = p->ring.ok ? DDSP_KERNEL_RING : p->tiled.ok ? DDSP_KERNEL_TILED : DDSP_KERNEL_DIRECT;
+        p->kernel = (p->ring.ok || p->ringx.ok) ? DDSP_KERNEL_RING : p->tiled.ok ? DDSP_KERNEL_TILED : DDSP_KERNEL_DIRECT;
     else
         p->kernel = p->kernel_req;
 }
@@ -153,6 +153,7 @@ int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, 
     }
     rc = ddsp_tiled_plan(p);
     if (rc == DDSP_OK) rc = ddsp_ring_plan(p);
+    if (rc == DDSP_OK) rc = ddsp_ringx_plan(p);
     if (rc != DDSP_OK) { ddsp_plan_destroy(p); return rc; }
     resolve_kernel(p);
     *plan = p;
@@ -165,8 +166,11 @@ int ddsp_plan_set_pitch(ddsp_plan* p, int64_t in_pitch, int64_t out_pitch) {
     p->out_pitch = out_pitch;
     if (p->d_stage_in) { cudaFree(p->d_stage_in); p->d_stage_in = nullptr; }
     if (p->d_stage_out) { cudaFree(p->d_stage_out); p->d_stage_out = nullptr; }
-    const int rc = ddsp_tiled_set_pitch(p);
-    return rc != DDSP_OK ? rc : ddsp_ring_set_pitch(p);
+    int rc = ddsp_tiled_set_pitch(p);
+    if (rc == DDSP_OK) rc = ddsp_ring_set_pitch(p);
+    if (rc == DDSP_OK) rc = ddsp_ringx_set_pitch(p);
+    resolve_kernel(p);     // a pitch can disable a kernel that AUTO had chosen (16-byte row alignment)
+    return rc;
 }
 
 int ddsp_plan_set_kernel(ddsp_plan* p, int kernel) {
@@ -175,7 +179,7 @@ int ddsp_plan_set_kernel(ddsp_plan* p, int kernel) {
         kernel != DDSP_KERNEL_RING)
         return DDSP_ERR_INVALID_ARG;
     if (kernel == DDSP_KERNEL_TILED && !p->tiled.ok) return DDSP_ERR_UNSUPPORTED;
-    if (kernel == DDSP_KERNEL_RING && !p->ring.ok) return DDSP_ERR_UNSUPPORTED;
+    if (kernel == DDSP_KERNEL_RING && !p->ring.ok && !p->ringx.ok) return DDSP_ERR_UNSUPPORTED;
     p->kernel_req = kernel;
     resolve_kernel(p);
     return DDSP_OK;
@@ -201,6 +205,7 @@ int ddsp_execute(const ddsp_plan* p, const void* d_in, void* d_out, void* cuda_s
     cudaError_t e;
     if (p->kernel == DDSP_KERNEL_RING) {
         if (ddsp_ring_can_run(p, d_in, d_out)) e = ddsp_launch_ring(p, d_in, d_out, s);
+        else if (ddsp_ringx_can_run(p, d_in, d_out)) e = ddsp_launch_ringx(p, d_in, d_out, s);
         else if (p->kernel_req == DDSP_KERNEL_RING) return DDSP_ERR_UNSUPPORTED;
         // unaligned input base: correct through the register-staged or the direct kernel
         else if (ddsp_tiled_can_run(p, d_in, d_out)) e = ddsp_launch_tiled(p, d_in, d_out, s);
@@ -241,6 +246,7 @@ int ddsp_plan_destroy(ddsp_plan* p) {
     if (!p) return DDSP_OK;
     ddsp_tiled_free(p);
     ddsp_ring_free(p);
+    ddsp_ringx_free(p);
     if (p->d_delays) cudaFree(p->d_delays);
     if (p->d_chan_list) cudaFree(p->d_chan_list);
     if (p->d_stage_in) cudaFree(p->d_stage_in);
