@@ -242,7 +242,7 @@ def run_ours(args):
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved / 1e9, "peak": p_add / 1e9, "unit": "Gadd/s",
                          "frac": achieved / p_add, "traffic": args.traffic_bytes,
-                         "peak_source": "148 SM x 128 int32 adds/clk/SM (measured, profiles/ubench_r01.md) x 1965 MHz",
+                         "peak_source": "148 SM x 128 int32 adds/clk/SM (measured, profiles/ubench_r01_raw.txt) x 1965 MHz",
                          "kernel_ms": launch_s * 1e3,
                          "t_roof_ms": t_roof * 1e3, "frac_of_path_roofline": t_roof / (secs / args.steps),
                          "hbm_ideal_bytes": ideal_bytes, "hbm_peak_gbs": hbm / 1e9,

@@ -80,7 +80,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ring_u8_kernel(const RingArg
     const int blk = blockIdx.x % a.nblk;
     const int64_t t0 = (int64_t)(blockIdx.x / a.nblk) * kTileT;
     const int NS = a.nstage, S = a.row_stride;
-    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t smem_base = smem_addr(smem);
     const uint32_t rows_bytes = (uint32_t)(C * 4 * S);   // the table of a stage follows its rows
 
     auto bar_raw = [&](int s) { return smem_base + (uint32_t)s * 8u; };
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ring_u8_kernel(const RingArg
             mbar_init(bar_raw(s), 1);
             mbar_init(bar_built(s), kWarps);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_barrier_init();
     }
     __syncthreads();
 
@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ring_u8_kernel(const RingArg
             const int tail = room > 0 ? (int)(room - cp) : 0;
             for (int i = 0; i < tail; ++i) smem[kBarBytes + (size_t)s * a.stage_bytes + (size_t)lane * 4 * S + cp + i] = a.in[so + cp + i];
             // these generic-proxy writes precede later copy-engine writes to the same bytes
-            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            fence_proxy_async_smem();
         }
         uint32_t total = cp;
 #pragma unroll

@@ -59,7 +59,7 @@ __device__ __forceinline__ void issue_chunk(const RingXArgs& a, uint8_t* smem, i
         const int tail = room > 0 ? (int)(room - cp) : 0;
         for (int i = 0; i < tail; ++i)
             smem[kBarBytes + (size_t)slot * a.raw_slot_bytes + (size_t)lane * a.raw_stride + cp + i] = a.in[so + cp + i];
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        fence_proxy_async_smem();
     }
     uint32_t total = cp;
 #pragma unroll
@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringf_kernel(const RingXArgs
     const int blk = blockIdx.x % a.nblk;
     const int64_t t0 = (int64_t)(blockIdx.x / a.nblk) * kTileF;
     const int NS = a.nraw;
-    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t smem_base = smem_addr(smem);
     const uint32_t rows_bytes = (uint32_t)(C * a.raw_stride);
 
     auto bar_raw = [&](int s) { return smem_base + (uint32_t)s * 8u; };
@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringf_kernel(const RingXArgs
             mbar_init(bar_raw(s), 1);
             mbar_init(bar_built(s), kWarps);
         }
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_barrier_init();
     }
     __syncthreads();
 
@@ -185,12 +185,6 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringf_kernel(const RingXArgs
 // bin slot when every warp is past the hot loop of its chunk.
 // Table of a chunk: C x 32 byte offsets ((slot * 2 + (q & 1)) * bins_stride + (q >> 1) * 4), C counts of 8-bin
 // units to form, C raw byte indices (within the channel row) of the window start at tile 0.
-__device__ __forceinline__ uint32_t lds8(uint32_t addr) {
-    uint32_t v;
-    asm volatile("ld.shared.u8 %0, [%1];" : "=r"(v) : "r"(addr));
-    return v;
-}
-
 // DS: compile-time downsample factor of the fast binning paths (2, 4), 0 = any factor (byte loop)
 template <int BDM_T, int KWT, int C, int DS>
 __global__ void __launch_bounds__(kThreads, 1) ddsp_ringb_kernel(const RingXArgs a) {
@@ -204,7 +198,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringb_kernel(const RingXArgs
     const int64_t t0 = (int64_t)(blockIdx.x / a.nblk) * kTileB;
     const int NR = a.nraw, NB = a.nbins, ds = DS ? DS : a.ds;
     const int Sr = a.raw_stride, Sb = a.bins_stride;
-    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t smem_base = smem_addr(smem);
     const uint32_t raw_rows_bytes = (uint32_t)(C * Sr), bin_rows_bytes = (uint32_t)(C * 2 * Sb);
 
     auto bar_raw = [&](int s) { return smem_base + (uint32_t)s * 8u; };
@@ -217,7 +211,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringb_kernel(const RingXArgs
     if (tid == 0) {
         for (int s = 0; s < NR; ++s) mbar_init(bar_raw(s), 1);
         for (int s = 0; s < NB; ++s) mbar_init(bar_built(s), kWarps);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_barrier_init();
     }
     __syncthreads();
 
@@ -252,7 +246,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringb_kernel(const RingXArgs
         // the offsets of the chunk move to the bin slot: the raw slot is refilled before the hot loop runs
         if (tid < C * kBdm) {
             const uint32_t v = lds32(tb + (uint32_t)tid * 4u);
-            asm volatile("st.shared.u32 [%0], %1;" ::"r"(bs + bin_rows_bytes + (uint32_t)tid * 4u), "r"(v) : "memory");
+            sts32(bs + bin_rows_bytes + (uint32_t)tid * 4u, v);
         }
         uint32_t total = 0;
 #pragma unroll

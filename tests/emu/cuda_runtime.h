@@ -1,0 +1,97 @@
+// Fake <cuda_runtime.h> of the CPU emulation harness (tests/emu): just enough of the CUDA runtime API and
+// of the device-side keywords for the ring kernels' sources (paper_2511_02328_b200/csrc/ddsp_ring*.cu and
+// ddsp_plan.cpp) to compile with g++ and run with one std::thread per CUDA thread.  Test infrastructure
+// only: nothing in the product includes this file.  "Device memory" is host memory.
+#pragma once
+
+#include <cstddef>
+#include <cstdint>
+#include <cstdlib>
+#include <cstring>
+#include <functional>
+
+// ---- keywords --------------------------------------------------------------------------------------
+#define __global__
+#define __device__
+#define __host__
+#define __forceinline__ inline
+#define __launch_bounds__(...)
+#define __align__(n)
+#define __grid_constant__
+
+// ---- vector types ----------------------------------------------------------------------------------
+struct uint2 { unsigned x, y; };
+struct uint3 { unsigned x, y, z; };
+struct uint4 { unsigned x, y, z, w; };
+inline uint2 make_uint2(unsigned x, unsigned y) { return uint2{x, y}; }
+inline uint4 make_uint4(unsigned x, unsigned y, unsigned z, unsigned w) { return uint4{x, y, z, w}; }
+
+// ---- runtime API -----------------------------------------------------------------------------------
+typedef int cudaError_t;
+enum { cudaSuccess = 0, cudaErrorMemoryAllocation = 2, cudaErrorInvalidConfiguration = 9 };
+enum cudaMemcpyKind { cudaMemcpyHostToDevice = 1, cudaMemcpyDeviceToHost = 2 };
+enum cudaFuncAttribute { cudaFuncAttributeMaxDynamicSharedMemorySize = 8 };
+typedef void* cudaStream_t;
+struct cudaDeviceProp { int multiProcessorCount; size_t sharedMemPerBlockOptin; };
+
+inline cudaError_t cudaGetDevice(int* d) { *d = 0; return cudaSuccess; }
+inline cudaError_t cudaGetDeviceProperties(cudaDeviceProp* p, int) {
+    p->multiProcessorCount = 148;
+    p->sharedMemPerBlockOptin = 232448;
+    return cudaSuccess;
+}
+inline cudaError_t cudaMalloc(void** p, size_t n) { *p = std::malloc(n ? n : 1); return *p ? cudaSuccess : cudaErrorMemoryAllocation; }
+inline cudaError_t cudaFree(void* p) { std::free(p); return cudaSuccess; }
+inline cudaError_t cudaMemcpy(void* d, const void* s, size_t n, cudaMemcpyKind) { std::memcpy(d, s, n); return cudaSuccess; }
+inline cudaError_t cudaMemcpyAsync(void* d, const void* s, size_t n, cudaMemcpyKind, cudaStream_t) { std::memcpy(d, s, n); return cudaSuccess; }
+inline cudaError_t cudaMemcpy2DAsync(void* d, size_t dp, const void* s, size_t sp, size_t w, size_t h, cudaMemcpyKind, cudaStream_t) {
+    for (size_t r = 0; r < h; ++r) std::memcpy((char*)d + r * dp, (const char*)s + r * sp, w);
+    return cudaSuccess;
+}
+inline cudaError_t cudaStreamSynchronize(cudaStream_t) { return cudaSuccess; }
+inline cudaError_t cudaGetLastError() { return cudaSuccess; }
+template <class F> cudaError_t cudaFuncSetAttribute(F, cudaFuncAttribute, int) { return cudaSuccess; }
+
+// ---- the emulated CTA (emu_runtime.cpp) ------------------------------------------------------------
+namespace emu {
+struct Ctx { unsigned tid, bid; };
+extern thread_local Ctx ctx;
+uint8_t* smem();                                   // dynamic shared memory of the running CTA
+void launch(unsigned grid, unsigned nthreads, size_t smem_bytes, const std::function<void()>& body);
+void syncthreads();
+void syncwarp();
+unsigned shfl_xor(unsigned v, int lane_mask);
+}  // namespace emu
+
+struct EmuIdx { unsigned x; };
+#define threadIdx (EmuIdx{emu::ctx.tid})
+#define blockIdx (EmuIdx{emu::ctx.bid})
+
+template <class F, class A>
+void emu_launch(F fn, unsigned grid, unsigned nthreads, size_t smem_bytes, cudaStream_t, const A& a) {
+    emu::launch(grid, nthreads, smem_bytes, [&]() { fn(a); });
+}
+
+// ---- device intrinsics -----------------------------------------------------------------------------
+inline void __syncthreads() { emu::syncthreads(); }
+inline void __syncwarp() { emu::syncwarp(); }
+inline unsigned __shfl_xor_sync(unsigned, unsigned v, int m) { return emu::shfl_xor(v, m); }
+template <class T> inline T __ldg(const T* p) { return *p; }
+inline int min(int a, int b) { return a < b ? a : b; }
+inline unsigned __byte_perm(unsigned x, unsigned y, unsigned s) {       // PTX prmt, default mode
+    const uint64_t src = ((uint64_t)y << 32) | x;
+    unsigned r = 0;
+    for (int i = 0; i < 4; ++i) {
+        const unsigned sel = (s >> (4 * i)) & 0xf;
+        unsigned b = (unsigned)(src >> (8 * (sel & 7))) & 0xff;
+        if (sel & 8) b = (b & 0x80) ? 0xff : 0x00;
+        r |= b << (8 * i);
+    }
+    return r;
+}
+inline unsigned __dp4a(unsigned a, unsigned b, unsigned c) {
+    for (int i = 0; i < 4; ++i) c += ((a >> (8 * i)) & 0xff) * ((b >> (8 * i)) & 0xff);
+    return c;
+}
+inline float __fadd_rn(float a, float b) { return a + b; }
+inline float __uint_as_float(unsigned u) { float f; std::memcpy(&f, &u, 4); return f; }
