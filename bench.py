@@ -147,6 +147,45 @@ def time_oracle(wl, rows, ncol, xh, dmax):
 
 
 # ----------------------------------------------------------------------------------------------
+# kernel gate: the ring kernels are opt-in in the library until they have passed their parity tests on
+# the GPU at hand.  bench.py runs exactly those tests (oracle comparison through the C ABI) in a child
+# process with a time limit and opts in only if every one of them passes; the outcome is reported in
+# config.ring_gate.  A crash or a hang of the child cannot take the benchmark down.
+# ----------------------------------------------------------------------------------------------
+def ring_gate(timeout_s=420):
+    if os.environ.get("DDSP_ENABLE_RING") is not None:
+        return os.environ["DDSP_ENABLE_RING"] not in ("", "0"), "preset by DDSP_ENABLE_RING"
+    cmd = [sys.executable, "-m", "pytest", os.path.join(ROOT, "tests", "test_parity_gpu.py"), "-m", "gpu", "-x", "-q",
+           "-k", "ring", "-p", "no:cacheprovider"]
+    try:
+        r = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, DDSP_ENABLE_RING="1"), capture_output=True, text=True,
+                           timeout=timeout_s)
+    except subprocess.TimeoutExpired:
+        return False, "parity tests of the ring kernels timed out after %d s" % timeout_s
+    tail = (r.stdout.strip().splitlines() or [""])[-1]
+    ok = r.returncode == 0 and " passed" in tail and "failed" not in tail and "error" not in tail
+    return ok, ("passed: " if ok else "FAILED (rc %d): " % r.returncode) + tail
+
+
+def time_kernel(plan, x, out, stream, kernel, steps=2):
+    """ms per execute of one kernel of the plan (1 warm-up), or None if it cannot run the plan."""
+    import torch
+    from paper_2511_02328_b200 import binding
+    try:
+        plan.set_kernel(kernel)
+    except binding.DdspError:
+        return None
+    plan.execute(x, out, stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        plan.execute(x, out, stream)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / steps
+
+
+# ----------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -171,6 +210,20 @@ def run_ours(args):
     unit = list(multi.shard_units(world, rank, world))[0]
     wl.seed = wl.seed + 1000 * unit
 
+    gate_note = None
+    if args.kernel == "auto":
+        # rank 0 decides; the other ranks read its decision after the barrier
+        flag = os.path.join("/tmp", "ddsp_ring_gate_%s" % os.environ.get("MASTER_PORT", str(os.getpid())))
+        if rank == 0:
+            ok, gate_note = ring_gate()
+            with open(flag, "w") as f:
+                f.write("1" if ok else "0")
+        multi.barrier()
+        if open(flag).read().strip() == "1":
+            os.environ["DDSP_ENABLE_RING"] = "1"
+        multi.barrier()
+        if rank == 0:
+            os.remove(flag)
     plan = binding.plan_for(wl)
     in_pitch = synth.round_up(wl.nsamp, 128)
     out_pitch = synth.round_up(plan.nsamp_out, 32)
@@ -182,6 +235,16 @@ def run_ours(args):
                       device=dev)
     stream = torch.cuda.current_stream(dev)
     adds = adds_per_execute(plan)
+    if args.kernel == "auto" and os.environ.get("DDSP_ENABLE_RING") == "1":
+        # both tiled kernels are verified here: run the faster one (measured on this workload)
+        t_ring = time_kernel(plan, x, out, stream, binding.DDSP_KERNEL_RING)
+        t_tiled = time_kernel(plan, x, out, stream, binding.DDSP_KERNEL_TILED)
+        pick = binding.DDSP_KERNEL_RING if t_ring is not None and (t_tiled is None or t_ring <= t_tiled) else \
+            (binding.DDSP_KERNEL_TILED if t_tiled is not None else binding.DDSP_KERNEL_AUTO)
+        plan.set_kernel(pick)
+        if gate_note is not None:
+            gate_note += "; ms per execute: ring %s, tiled %s" % (
+                "%.1f" % t_ring if t_ring else "n/a", "%.1f" % t_tiled if t_tiled else "n/a")
 
     for _ in range(max(args.warmup, 0)):
         plan.execute(x, out, stream)
@@ -235,6 +298,7 @@ def run_ours(args):
                        "nsamp": wl.nsamp, "nsamp_out": plan.nsamp_out, "tsamp_s": wl.tsamp,
                        "downsample": wl.downsample, "in_dtype": wl.dtype,
                        "kernel": {1: "direct", 2: "tiled", 3: "ring"}[plan.kernel],
+                       "ring_gate": gate_note,
                        "units": "one observation per GPU", "parallelism": "dp%d" % world,
                        "l2": "inputs (%.2f GB) larger than L2; no flush" % (x.numel() * x.element_size() / 1e9)},
             "x_realtime": plan.nsamp_out * wl.tsamp * wl.downsample / (t_max / args.steps),
