@@ -346,12 +346,23 @@ def measure_e2e(plan, wl, x, out, in_pitch, out_pitch, adds, steps, multi):
     xh = torch.empty(x.shape, dtype=x.dtype, pin_memory=True)
     xh.copy_(x)
     oh = torch.empty(out.shape, dtype=out.dtype, pin_memory=True)
-    plan.execute_host(xh, oh)                      # warm-up: allocates the staging buffers
+    from paper_2511_02328_b200 import binding
+    call, how = plan.execute_host, "ddsp_execute_host (copy in, kernel, copy out in sequence)"
+    if plan.kernel == binding.DDSP_KERNEL_RING:
+        # the ring kernels can run on a range of time tiles: overlap copy-in, kernel and copy-out
+        try:
+            plan.execute_host_pipelined(xh, oh, nchunks=16)
+            if torch.equal(oh[:, :plan.nsamp_out], out[:, :plan.nsamp_out].cpu()):
+                call = lambda a, b: plan.execute_host_pipelined(a, b, nchunks=16)
+                how = "ddsp_execute_host_pipelined (16 pieces, copies and kernels overlapped)"
+        except binding.DdspError:
+            pass
+    call(xh, oh)                                   # warm-up: allocates the staging buffers
     torch.cuda.synchronize()
     multi.barrier()
     t0 = time.perf_counter()
     for _ in range(steps):
-        plan.execute_host(xh, oh)                  # synchronises the stream before returning
+        call(xh, oh)                               # synchronises before returning
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     rate, t_max = multi.job_throughput(adds * steps, dt)
@@ -359,7 +370,7 @@ def measure_e2e(plan, wl, x, out, in_pitch, out_pitch, adds, steps, multi):
     return {"value": rate / 1e9, "unit": UNIT, "h2d_bytes_per_step": in_bytes,
             "d2h_bytes_per_step": valid_out_bytes, "steps": steps, "ms_per_step": t_max / steps * 1e3,
             "x_realtime": plan.nsamp_out * wl.tsamp * wl.downsample / (t_max / steps),
-            "matches_device_result": same}
+            "matches_device_result": same, "call": how}
 
 
 # ----------------------------------------------------------------------------------------------

@@ -104,6 +104,17 @@ DDSP_API int ddsp_execute(const ddsp_plan* plan, const void* d_in, void* d_out, 
  * h_out: ndm rows of out_pitch elements.  Not re-entrant for one plan (the staging buffers are shared). */
 DDSP_API int ddsp_execute_host(ddsp_plan* plan, const void* h_in, void* h_out, void* cuda_stream);
 
+/* ddsp_execute_host with the three phases overlapped (the paper names the copies, not the kernel, as its
+ * bottleneck and leaves their overlap undone): the output columns are cut into
+ * nchunks pieces (multiples of 2048 samples); piece j needs input columns < (end_j + d_max) * ds only, so
+ * the copy of the input for piece j+1, the kernel of piece j and the copy of piece j-1's result run at the
+ * same time on three internal streams.  Same buffers, layout and result as ddsp_execute_host; synchronises
+ * cuda_stream first and returns when everything is done.  Pinned host memory is needed for real overlap.
+ * DDSP_ERR_UNSUPPORTED unless the plan runs a ring kernel (DDSP_KERNEL_RING: the only kernels that can be
+ * launched on a range of time tiles). */
+DDSP_API int ddsp_execute_host_pipelined(ddsp_plan* plan, const void* h_in, void* h_out, void* cuda_stream,
+                                         int nchunks);
+
 /* Introspection of the ring kernel's plan-time tables (tile geometry; DESIGN.md section
  * 6), so that the host logic can be tested without a GPU.  DDSP_ERR_UNSUPPORTED if the ring kernel cannot
  * run this plan.  geom: host int32[10] = {rows per stage C, DM blocks, chunks, padded channel count,

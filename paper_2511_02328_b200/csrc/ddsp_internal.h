@@ -105,6 +105,8 @@ struct ddsp_plan {
     // staging buffers of ddsp_execute_host
     void* d_stage_in = nullptr;
     void* d_stage_out = nullptr;
+    // streams of ddsp_execute_host_pipelined (created on first use)
+    cudaStream_t hs_in = nullptr, hs_k = nullptr, hs_out = nullptr;
 };
 
 // ddsp_direct.cu
@@ -124,11 +126,14 @@ int ddsp_ring_plan(ddsp_plan* p);
 int ddsp_ring_set_pitch(ddsp_plan* p);    // rebuilds the pitch-dependent tables
 void ddsp_ring_free(ddsp_plan* p);
 bool ddsp_ring_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);   // 16-byte aligned input base
-cudaError_t ddsp_launch_ring(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);
+// tile0 / ntile: range of time tiles (of the kernel's tile length) to compute; ntile < 0 = all from tile0 on
+cudaError_t ddsp_launch_ring(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s, int64_t tile0 = 0,
+                             int64_t ntile = -1);
 
 // ddsp_ringx.cu (same entry points as the ring kernel, for float32 and for uint8 with ds > 1)
 int ddsp_ringx_plan(ddsp_plan* p);
 int ddsp_ringx_set_pitch(ddsp_plan* p);
 void ddsp_ringx_free(ddsp_plan* p);
 bool ddsp_ringx_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);
-cudaError_t ddsp_launch_ringx(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);
+cudaError_t ddsp_launch_ringx(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s, int64_t tile0 = 0,
+                              int64_t ntile = -1);

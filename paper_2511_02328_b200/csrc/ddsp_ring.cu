@@ -60,6 +60,7 @@ struct RingArgs {
     const uint32_t* tbl;      // [nblk][nchunk][tblw]: C x 32 stage-relative byte offsets, then C unit counts, padding
     const int32_t* rows;      // [nblk * 32] output row of each sorted trial, -1 = padding
     int64_t out_pitch, nsamp_out, in_valid;   // in_valid: bytes of the input buffer that may be read
+    int64_t tile0;            // first time tile of this launch (a launch may cover a range of tiles)
     int nlist, nch_pad, nblk, nchunk, row_stride, stage_bytes, nstage, tblw, out_vec;
     uint32_t one;             // 1: multiplier that routes an add through the FMA pipe (IMAD)
 };
@@ -78,7 +79,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ring_u8_kernel(const RingArg
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slab = warp % SLABS, grp = warp / SLABS;
     const int blk = blockIdx.x % a.nblk;
-    const int64_t t0 = (int64_t)(blockIdx.x / a.nblk) * kTileT;
+    const int64_t t0 = ((int64_t)(blockIdx.x / a.nblk) + a.tile0) * kTileT;
     const int NS = a.nstage, S = a.row_stride;
     const uint32_t smem_base = smem_addr(smem);
     const uint32_t rows_bytes = (uint32_t)(C * 4 * S);   // the table of a stage follows its rows
@@ -442,7 +443,8 @@ bool ddsp_ring_can_run(const ddsp_plan* p, const void* d_in, const void* d_out) 
     return p->ring.ok && d_in != nullptr && d_out != nullptr && ((uintptr_t)d_in % 16 == 0);
 }
 
-cudaError_t ddsp_launch_ring(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s) {
+cudaError_t ddsp_launch_ring(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s, int64_t tile0,
+                             int64_t ntile) {
     const ddsp_ring& g = p->ring;
     RingArgs a;
     a.in = (const uint8_t*)d_in;
@@ -453,7 +455,10 @@ cudaError_t ddsp_launch_ring(const ddsp_plan* p, const void* d_in, void* d_out, 
     a.nlist = (int)p->chan_list.size(); a.nch_pad = g.nch_pad; a.nblk = g.nblk; a.nchunk = g.nchunk;
     a.row_stride = g.row_stride; a.stage_bytes = g.stage_bytes; a.nstage = g.nstage; a.tblw = g.tblw;
     a.out_vec = ((uintptr_t)d_out % 16 == 0) && (p->out_pitch % 4 == 0);
-    const unsigned grid = (unsigned)(g.ntile_t * g.nblk);
+    if (ntile < 0) ntile = g.ntile_t - tile0;          // default: every tile from tile0 on
+    if (tile0 < 0 || ntile < 1 || tile0 + ntile > g.ntile_t) return cudaErrorInvalidConfiguration;
+    a.tile0 = tile0;
+    const unsigned grid = (unsigned)(ntile * g.nblk);
     kVariants[g.variant].fn<<<grid, kThreads, g.smem_bytes, s>>>(a);
     return cudaGetLastError();
 }

@@ -41,6 +41,7 @@ struct RingXArgs {
     const uint32_t* tbl;      // [nblk][nchunk][tblw]
     const int32_t* rows;      // [nblk * 32]
     int64_t out_pitch, nsamp_out, in_valid, nsamp;
+    int64_t tile0;            // first time tile of this launch
     int nlist, nch_pad, nblk, nchunk, raw_stride, bins_stride, raw_slot_bytes, bins_slot_bytes, nraw, nbins;
     int tblw, ds, flush_every, out_vec;
 };
@@ -85,7 +86,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringf_kernel(const RingXArgs
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slab = warp % SLABS, grp = warp / SLABS;
     const int blk = blockIdx.x % a.nblk;
-    const int64_t t0 = (int64_t)(blockIdx.x / a.nblk) * kTileF;
+    const int64_t t0 = ((int64_t)(blockIdx.x / a.nblk) + a.tile0) * kTileF;
     const int NS = a.nraw;
     const uint32_t smem_base = smem_addr(smem);
     const uint32_t rows_bytes = (uint32_t)(C * a.raw_stride);
@@ -195,7 +196,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringb_kernel(const RingXArgs
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slab = warp % SLABS, grp = warp / SLABS;
     const int blk = blockIdx.x % a.nblk;
-    const int64_t t0 = (int64_t)(blockIdx.x / a.nblk) * kTileB;
+    const int64_t t0 = ((int64_t)(blockIdx.x / a.nblk) + a.tile0) * kTileB;
     const int NR = a.nraw, NB = a.nbins, ds = DS ? DS : a.ds;
     const int Sr = a.raw_stride, Sb = a.bins_stride;
     const uint32_t smem_base = smem_addr(smem);
@@ -597,7 +598,8 @@ bool ddsp_ringx_can_run(const ddsp_plan* p, const void* d_in, const void* d_out)
     return p->ringx.ok && d_in != nullptr && d_out != nullptr && ((uintptr_t)d_in % 16 == 0);
 }
 
-cudaError_t ddsp_launch_ringx(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s) {
+cudaError_t ddsp_launch_ringx(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s, int64_t tile0,
+                              int64_t ntile) {
     const ddsp_ringx& g = p->ringx;
     const int64_t esize = g.kind == 2 ? 4 : 1;
     RingXArgs a;
@@ -611,7 +613,10 @@ cudaError_t ddsp_launch_ringx(const ddsp_plan* p, const void* d_in, void* d_out,
     a.raw_slot_bytes = g.raw_slot_bytes; a.bins_slot_bytes = g.bins_slot_bytes; a.nraw = g.nraw; a.nbins = g.nbins;
     a.tblw = g.tblw; a.ds = p->ds; a.flush_every = g.flush_every;
     a.out_vec = ((uintptr_t)d_out % 8 == 0) && (p->out_pitch % 2 == 0);
-    const unsigned grid = (unsigned)(g.ntile_t * g.nblk);
+    if (ntile < 0) ntile = g.ntile_t - tile0;
+    if (tile0 < 0 || ntile < 1 || tile0 + ntile > g.ntile_t) return cudaErrorInvalidConfiguration;
+    a.tile0 = tile0;
+    const unsigned grid = (unsigned)(ntile * g.nblk);
     kVariants[g.variant].fn<<<grid, kThreads, g.smem_bytes, s>>>(a);
     return cudaGetLastError();
 }

@@ -47,7 +47,7 @@ def aligned(shape, dtype, fill=None):
     return a
 
 
-def run_emulated(emu, wl, x, in_pitch, kernel=binding.DDSP_KERNEL_RING):
+def run_emulated(emu, wl, x, in_pitch, kernel=binding.DDSP_KERNEL_RING, host_chunks=0):
     dm = np.ascontiguousarray(wl.dm_list, dtype=np.float64)
     mask = None if wl.mask is None else np.ascontiguousarray(wl.mask, dtype=np.uint8)
     h = ctypes.c_void_p()
@@ -64,7 +64,10 @@ def run_emulated(emu, wl, x, in_pitch, kernel=binding.DDSP_KERNEL_RING):
         xin[...] = x
         out = aligned((wl.ndm, out_pitch), np.uint32 if wl.dtype == "u8" else np.float32, fill=7)
         f0 = emu.ddsp_emu_faults()
-        rc = emu.ddsp_execute(h, xin.ctypes.data, out.ctypes.data, None)
+        if host_chunks:      # the overlapped host-buffer path: device staging buffers, pieces of the output columns
+            rc = emu.ddsp_execute_host_pipelined(h, xin.ctypes.data, out.ctypes.data, None, host_chunks)
+        else:
+            rc = emu.ddsp_execute(h, xin.ctypes.data, out.ctypes.data, None)
         assert rc == 0, rc
         assert emu.ddsp_emu_faults() == f0, "the emulator flagged a fault (see stderr)"
         assert (out[:, nout:] == 7).all(), "pitch padding was written"
@@ -73,10 +76,10 @@ def run_emulated(emu, wl, x, in_pitch, kernel=binding.DDSP_KERNEL_RING):
         emu.ddsp_plan_destroy(h)
 
 
-def check(emu, oracle, wl, pitch=None):
+def check(emu, oracle, wl, pitch=None, host_chunks=0):
     from _util import make_input
     x = make_input(oracle, wl, "cpu", pitch=pitch).numpy()
-    got, nout = run_emulated(emu, wl, x, x.shape[1])
+    got, nout = run_emulated(emu, wl, x, x.shape[1], host_chunks=host_chunks)
     want, nout_o, _ = oracle.dedisperse(x, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, nsamp=wl.nsamp,
                                         downsample=wl.downsample, mask=wl.mask)
     assert nout == nout_o
@@ -124,6 +127,26 @@ def test_f32_ring(emu, oracle, pitch):
                         mean=0.0, std=1.0)
     wl.mask = (np.arange(19) % 5 == 3).astype(np.uint8)
     check(emu, oracle, wl, pitch)
+
+
+@pytest.mark.timeout(1200)
+@pytest.mark.parametrize("kind", ["u8", "bins4", "f32"])
+def test_host_pipelined_pieces(emu, oracle, kind):
+    """ddsp_execute_host_pipelined: three pieces of the output columns, each launched on its own range of time
+    tiles after only the input columns it needs (< (end + d_max) * ds) were copied; result equals the oracle."""
+    if kind == "u8":
+        wl = synth.Workload("emu-pipe-u8", 31, 9, 1400.0, -8.0, 2e-4, 6000, np.linspace(0, 200, 33), dtype="u8",
+                            mean=128.0, std=60.0)
+        pitch = 6016
+    elif kind == "bins4":
+        wl = synth.Workload("emu-pipe-b4", 32, 9, 1400.0, -8.0, 1e-4, 4 * 6000 + 2, np.linspace(0, 100, 20),
+                            downsample=4, dtype="u8", mean=200.0, std=50.0)
+        pitch = synth.round_up(wl.nsamp, 16)
+    else:
+        wl = synth.Workload("emu-pipe-f32", 33, 9, 800.0, -8.0, 5e-4, 5000, np.linspace(0, 100, 20), dtype="f32",
+                            mean=0.0, std=1.0)
+        pitch = None
+    check(emu, oracle, wl, pitch, host_chunks=3)
 
 
 # ------------------------------------------------------------------------------------------------
