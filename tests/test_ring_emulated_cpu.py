@@ -102,6 +102,18 @@ def test_u8_ring_small(emu, oracle, pitch):
 
 
 @pytest.mark.timeout(900)
+@pytest.mark.parametrize("variant", range(1, 8))
+def test_u8_ring_variants(emu, oracle, variant, monkeypatch):
+    """Every compiled instantiation (odd-byte adds on the ALU / FMA pipe, 8 x 4 or 4 x 8 words per thread, 2 or 4
+    rows per stage) computes the same result; 300 channels so that the ring wraps and the lanes are flushed."""
+    monkeypatch.setenv("DDSP_RING_VARIANT", str(variant))
+    wl = synth.Workload("emu-var", 25, 300, 1400.0, -0.5, 5e-4, 2100, np.linspace(0, 60, 9), dtype="u8",
+                        mean=200.0, std=60.0)
+    wl.mask = (np.arange(300) % 11 == 4).astype(np.uint8)
+    check(emu, oracle, wl, 2112)
+
+
+@pytest.mark.timeout(900)
 def test_u8_ring_flush(emu, oracle):
     """More than 256 channels of value 255: the 16-bit lanes are flushed and must not overflow (I10)."""
     wl = synth.Workload("emu-flush", 22, 300, 1400.0, -0.5, 5e-4, 2100, np.linspace(0, 60, 9), dtype="u8",
