@@ -142,17 +142,15 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ring_u8_kernel(const RingArg
         const int s = chunk % NS;
         const uint32_t sb = stage_base(s);
         mbar_wait(bar_raw(s), (uint32_t)(chunk / NS) & 1u);
-        uint32_t n[C];
-        if (C == 4) lds128(sb + rows_bytes + C * kBdm * 4, n);
-        else { n[0] = lds32(sb + rows_bytes + C * kBdm * 4); n[1] = lds32(sb + rows_bytes + C * kBdm * 4 + 4); }
-        uint32_t total = 0;
-#pragma unroll
-        for (int r = 0; r < C; ++r) total += n[r];
-        for (uint32_t f = tid; f < total; f += kThreads) {
-            uint32_t r = 0, u = f;
-#pragma unroll
-            for (int q = 0; q < C - 1; ++q)
-                if (r == (uint32_t)q && u >= n[q]) { u -= n[q]; r = q + 1; }
+        // row r of the chunk is expanded by threads [r * TPR, (r + 1) * TPR): whole warps per row, one
+        // 16-byte unit per thread and pass; the (partial) last pass falls on the first warps of the group
+        // in even chunks and on the last ones in odd chunks, so that no warp is always the slow one
+        constexpr uint32_t TPR = kThreads / C;
+        const uint32_t r = (uint32_t)tid / TPR;
+        const uint32_t n = lds32(sb + rows_bytes + (uint32_t)((C * kBdm) * 4) + r * 4u);
+        uint32_t u = (uint32_t)tid % TPR;
+        if (chunk & 1) u = TPR - 1u - u;
+        for (; u < n; u += TPR) {
             const uint32_t addr = sb + r * 4u * (uint32_t)S + u * 16u;
             uint32_t w[4];
             lds128(addr, w);
