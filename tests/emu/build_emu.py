@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_2511_02328_b200", "csrc")
 BUILD = os.path.join(HERE, "build")
-PRODUCT = ["ddsp_plan.cpp", "ddsp_ring.cu", "ddsp_ringx.cu"]
+PRODUCT = ["ddsp_plan.cpp", "ddsp_ring.cu", "ddsp_ringx.cu", "ddsp_tiled.cu"]
 LIB = os.path.join(BUILD, "libddsp_emu.so")
 TSAN_EXE = os.path.join(BUILD, "emu_tsan")
 
@@ -25,6 +25,13 @@ def transform(text):
     text, n1 = re.subn(r"(\w[\w\[\]\.]*)<<<\s*([^;]*?)\s*>>>\((\w+)\);", r"emu_launch(\1, \2, \3);", text)
     text, n2 = re.subn(r"extern __shared__ __align__\(\d+\) uint8_t smem\[\];", "uint8_t* const smem = emu::smem();", text)
     text = text.replace('#include "ddsp_ring_common.cuh"', '#include "emu_common.h"')
+    # ddsp_tiled.cu (the kernel already verified on hardware; here it calibrates the emulation) keeps its PTX
+    # helpers in the file: cut them out and use the same host stand-ins
+    m = re.search(r"__device__ __forceinline__ uint32_t lds32\(uint32_t addr\) \{.*?mad\.wide\.u32.*?\n\}\n", text, flags=re.S)
+    if m:
+        text = text[:m.start()] + "using namespace ddsp_dev;\n" + text[m.end():]
+        text = text.replace('#include "ddsp_internal.h"', '#include "ddsp_internal.h"\n#include "emu_common.h"', 1)
+        text = text.replace("(uint32_t)__cvta_generic_to_shared(smem)", "smem_addr(smem)")
     return text, n1, n2
 
 

@@ -29,6 +29,7 @@ inline void sts128(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d
     std::memcpy(emu::smem() + addr, v, 16);
 }
 inline void add_fma_pipe(uint32_t& acc, uint32_t v, uint32_t one) { acc += v * one; }
+inline void add_wide(uint64_t& acc, uint32_t v, uint32_t one) { acc += (uint64_t)v * one; }
 inline void mbar_init(uint32_t bar, int count) { emu::mbar_init(bar, count); }
 inline void mbar_arrive(uint32_t bar) { emu::mbar_arrive(bar, 0); }
 inline void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) { emu::mbar_arrive(bar, bytes); }

@@ -102,6 +102,22 @@ def test_u8_ring_small(emu, oracle, pitch):
 
 
 @pytest.mark.timeout(900)
+@pytest.mark.parametrize("pitch", [None, 2112])
+def test_calibration_tiled_kernel(emu, oracle, pitch):
+    """Calibration of the emulation: DDSP_KERNEL_TILED, whose parity is green on a B200, gives the oracle's result
+    here as well (dense odd pitch = its byte-gather staging path, aligned pitch = its vector path; 300 channels
+    = two flushes)."""
+    wl = synth.Workload("emu-tiled", 26, 300, 1400.0, -0.5, 5e-4, 2100, np.linspace(0, 60, 40), dtype="u8",
+                        mean=128.0, std=60.0)
+    wl.mask = (np.arange(300) % 9 == 5).astype(np.uint8)
+    from _util import make_input
+    x = make_input(oracle, wl, "cpu", pitch=pitch).numpy()
+    got, nout = run_emulated(emu, wl, x, x.shape[1], kernel=binding.DDSP_KERNEL_TILED)
+    want, _, _ = oracle.dedisperse(x, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, nsamp=wl.nsamp, mask=wl.mask)
+    assert np.array_equal(got, want)
+
+
+@pytest.mark.timeout(900)
 @pytest.mark.parametrize("variant", range(1, 8))
 def test_u8_ring_variants(emu, oracle, variant, monkeypatch):
     """Every compiled instantiation (odd-byte adds on the ALU / FMA pipe, 8 x 4 or 4 x 8 words per thread, 2 or 4
