@@ -238,25 +238,20 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_ringb_kernel(const RingXArgs
         const uint32_t rs = raw_base(chunk % NR), bs = bin_base(chunk % NB);
         mbar_wait(bar_raw(chunk % NR), (uint32_t)(chunk / NR) & 1u);
         const uint32_t tb = rs + raw_rows_bytes;
-        uint32_t n[C], js[C];
-#pragma unroll
-        for (int r = 0; r < C; ++r) {
-            n[r] = lds32(tb + (uint32_t)((C * kBdm + r) * 4));
-            js[r] = lds32(tb + (uint32_t)((C * kBdm + C + r) * 4));
-        }
+        // row r of the chunk is binned by threads [r * TPR, (r + 1) * TPR) (whole warps per row); the partial
+        // last pass alternates between the group's first and last warps so that no warp is always the slow one
+        constexpr uint32_t TPR = kThreads / C;
+        const uint32_t r = (uint32_t)tid / TPR;
+        const uint32_t n = lds32(tb + (uint32_t)((C * kBdm) * 4) + r * 4u);
+        const uint32_t j0 = lds32(tb + (uint32_t)((C * kBdm + C) * 4) + r * 4u);
         // the offsets of the chunk move to the bin slot: the raw slot is refilled before the hot loop runs
         if (tid < C * kBdm) {
             const uint32_t v = lds32(tb + (uint32_t)tid * 4u);
             sts32(bs + bin_rows_bytes + (uint32_t)tid * 4u, v);
         }
-        uint32_t total = 0;
-#pragma unroll
-        for (int r = 0; r < C; ++r) total += n[r];
-        for (uint32_t f = tid; f < total; f += kThreads) {
-            uint32_t r = 0, u = f, j0 = js[0];
-#pragma unroll
-            for (int q = 0; q < C - 1; ++q)
-                if (r == (uint32_t)q && u >= n[q]) { u -= n[q]; r = q + 1; j0 = js[q + 1]; }
+        uint32_t u = (uint32_t)tid % TPR;
+        if (chunk & 1) u = TPR - 1u - u;
+        for (; u < n; u += TPR) {
             const uint32_t rb = rs + r * (uint32_t)Sr + u * (uint32_t)(8 * ds);
             // raw bytes of this row at window index >= limit lie beyond nsamp: they count as zero
             const int64_t limit = a.nsamp - ((int64_t)j0 + t0 * ds) - (int64_t)u * (8 * ds);
