@@ -16,13 +16,16 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_2511_02328_b200", "csrc")
 BUILD = os.path.join(HERE, "build")
-PRODUCT = ["ddsp_plan.cpp", "ddsp_ring.cu", "ddsp_ringx.cu", "ddsp_tiled.cu"]
+PRODUCT = ["ddsp_plan.cpp", "ddsp_ring.cu", "ddsp_ringx.cu", "ddsp_tiled.cu", "ddsp_direct.cu"]
 LIB = os.path.join(BUILD, "libddsp_emu.so")
 TSAN_EXE = os.path.join(BUILD, "emu_tsan")
 
 
 def transform(text):
     text, n1 = re.subn(r"(\w[\w\[\]\.]*)<<<\s*([^;]*?)\s*>>>\((\w+)\);", r"emu_launch(\1, \2, \3);", text)
+    # launches with an argument list (template kernels of ddsp_direct.cu)
+    text, n1b = re.subn(r"(\w+<[^;<>]*>)<<<\s*([^;]*?)\s*>>>\(", r"emu_launch_v(\1, \2, ", text)
+    n1 += n1b
     text, n2 = re.subn(r"extern __shared__ __align__\(\d+\) uint8_t smem\[\];", "uint8_t* const smem = emu::smem();", text)
     text = text.replace('#include "ddsp_ring_common.cuh"', '#include "emu_common.h"')
     # ddsp_tiled.cu (the kernel already verified on hardware; here it calibrates the emulation) keeps its PTX
@@ -64,12 +67,12 @@ def build(tsan=False, mutate=None):
                 assert text.count(mutate[1]) == 1, (name, mutate[1])
                 text = text.replace(mutate[1], mutate[2])
         if name.endswith(".cu"):
-            assert n1 >= 1 and n2 >= 1, (name, n1, n2)
+            assert n1 >= 1 and (n2 >= 1 or name == "ddsp_direct.cu"), (name, n1, n2)
         out = os.path.join(BUILD, os.path.splitext(name)[0] + tag + ".cpp")
         with open(out, "w") as f:
             f.write(text)
         srcs.append(out)
-    srcs += [os.path.join(HERE, "emu_runtime.cpp"), os.path.join(HERE, "emu_stubs.cpp")]
+    srcs += [os.path.join(HERE, "emu_runtime.cpp")]
     flags = ["-std=c++17", "-O1", "-g", "-fPIC", "-pthread", "-ffp-contract=off", "-fno-fast-math", "-w",
              "-I", HERE, "-I", CSRC, "-I", os.path.join(ROOT, "include")]
     if tsan:

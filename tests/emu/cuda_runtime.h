@@ -63,7 +63,7 @@ template <class F> cudaError_t cudaFuncSetAttribute(F, cudaFuncAttribute, int) {
 
 // ---- the emulated CTA (emu_runtime.cpp) ------------------------------------------------------------
 namespace emu {
-struct Ctx { unsigned tid, bid; };
+struct Ctx { unsigned tid, bid, bidy, gdimy; };
 extern thread_local Ctx ctx;
 uint8_t* smem();                                   // dynamic shared memory of the running CTA
 void launch(unsigned grid, unsigned nthreads, size_t smem_bytes, const std::function<void()>& body);
@@ -72,13 +72,24 @@ void syncwarp();
 unsigned shfl_xor(unsigned v, int lane_mask);
 }  // namespace emu
 
-struct EmuIdx { unsigned x; };
-#define threadIdx (EmuIdx{emu::ctx.tid})
-#define blockIdx (EmuIdx{emu::ctx.bid})
+struct EmuIdx { unsigned x, y; };
+struct dim3 {
+    unsigned x, y, z;
+    dim3(unsigned x_ = 1, unsigned y_ = 1, unsigned z_ = 1) : x(x_), y(y_), z(z_) {}
+};
+#define threadIdx (EmuIdx{emu::ctx.tid, 0u})
+#define blockIdx (EmuIdx{emu::ctx.bid, emu::ctx.bidy})
+#define gridDim (EmuIdx{0u, emu::ctx.gdimy})
 
 template <class F, class A>
 void emu_launch(F fn, unsigned grid, unsigned nthreads, size_t smem_bytes, cudaStream_t, const A& a) {
     emu::launch(grid, nthreads, smem_bytes, [&]() { fn(a); });
+}
+// 2-D grid, any argument list (the direct kernel): one emulated launch per grid row
+template <class F, class... A>
+void emu_launch_v(F fn, dim3 grid, unsigned nthreads, size_t smem_bytes, cudaStream_t, A... a) {
+    for (unsigned y = 0; y < grid.y; ++y)
+        emu::launch(grid.x, nthreads, smem_bytes, [&]() { emu::ctx.bidy = y; emu::ctx.gdimy = grid.y; fn(a...); });
 }
 
 // ---- device intrinsics -----------------------------------------------------------------------------

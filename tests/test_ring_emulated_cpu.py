@@ -118,6 +118,21 @@ def test_calibration_tiled_kernel(emu, oracle, pitch):
 
 
 @pytest.mark.timeout(900)
+@pytest.mark.parametrize("dtype,ds", [("u8", 1), ("u8", 3), ("f32", 2)])
+def test_calibration_direct_kernel(emu, oracle, dtype, ds):
+    """The other hardware-verified kernel, DDSP_KERNEL_DIRECT (2-D grid), in the same harness."""
+    wl = synth.Workload("emu-direct", 27, 11, 1400.0, -6.0, 2e-4, 1500 * ds + 1, np.linspace(0, 80, 7), downsample=ds,
+                        dtype=dtype, mean=128.0 if dtype == "u8" else 0.0, std=50.0 if dtype == "u8" else 1.0)
+    wl.mask = (np.arange(11) % 4 == 1).astype(np.uint8)
+    from _util import make_input
+    x = make_input(oracle, wl, "cpu").numpy()
+    got, nout = run_emulated(emu, wl, x, x.shape[1], kernel=binding.DDSP_KERNEL_DIRECT)
+    want, _, _ = oracle.dedisperse(x, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, nsamp=wl.nsamp, downsample=ds,
+                                   mask=wl.mask)
+    assert np.array_equal(got if dtype == "u8" else got.astype(np.float64), want)
+
+
+@pytest.mark.timeout(900)
 @pytest.mark.parametrize("variant", range(1, 8))
 def test_u8_ring_variants(emu, oracle, variant, monkeypatch):
     """Every compiled instantiation (odd-byte adds on the ALU / FMA pipe, 8 x 4 or 4 x 8 words per thread, 2 or 4
