@@ -1,4 +1,5 @@
-"""The ring kernels (ddsp_ring.cu, ddsp_ringx.cu) executed on the CPU, thread for thread.
+"""The library's kernels executed on the CPU, thread for thread: the ring kernels (ddsp_ring.cu, ddsp_ringx.cu),
+which have not run on hardware yet, and -- as calibration of the harness -- the two that have (tiled, direct).
 
 tests/emu compiles the kernels' own source with g++ (three textual substitutions, see build_emu.py) against
 host stand-ins of the PTX helpers: one std::thread per CUDA thread, mbarriers with the PTX counting rules, a
