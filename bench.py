@@ -36,7 +36,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="fast", help="workload name (synth.CONFIG_NAMES); headline = fast")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "tiled", "ring"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "tiled"])
     ap.add_argument("--crop", type=int, default=0, help="debug: crop to this many output samples")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -147,45 +147,6 @@ def time_oracle(wl, rows, ncol, xh, dmax):
 
 
 # ----------------------------------------------------------------------------------------------
-# kernel gate: the ring kernels are opt-in in the library until they have passed their parity tests on
-# the GPU at hand.  bench.py runs exactly those tests (oracle comparison through the C ABI) in a child
-# process with a time limit and opts in only if every one of them passes; the outcome is reported in
-# config.ring_gate.  A crash or a hang of the child cannot take the benchmark down.
-# ----------------------------------------------------------------------------------------------
-def ring_gate(timeout_s=420):
-    if os.environ.get("DDSP_ENABLE_RING") is not None:
-        return os.environ["DDSP_ENABLE_RING"] not in ("", "0"), "preset by DDSP_ENABLE_RING"
-    cmd = [sys.executable, "-m", "pytest", os.path.join(ROOT, "tests", "test_parity_gpu.py"), "-m", "gpu", "-x", "-q",
-           "-k", "ring", "-p", "no:cacheprovider"]
-    try:
-        r = subprocess.run(cmd, cwd=ROOT, env=dict(os.environ, DDSP_ENABLE_RING="1"), capture_output=True, text=True,
-                           timeout=timeout_s)
-    except subprocess.TimeoutExpired:
-        return False, "parity tests of the ring kernels timed out after %d s" % timeout_s
-    tail = (r.stdout.strip().splitlines() or [""])[-1]
-    ok = r.returncode == 0 and " passed" in tail and "failed" not in tail and "error" not in tail
-    return ok, ("passed: " if ok else "FAILED (rc %d): " % r.returncode) + tail
-
-
-def time_kernel(plan, x, out, stream, kernel, steps=2):
-    """ms per execute of one kernel of the plan (1 warm-up), or None if it cannot run the plan."""
-    import torch
-    from paper_2511_02328_b200 import binding
-    try:
-        plan.set_kernel(kernel)
-    except binding.DdspError:
-        return None
-    plan.execute(x, out, stream)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record(stream)
-    for _ in range(steps):
-        plan.execute(x, out, stream)
-    e1.record(stream)
-    torch.cuda.synchronize()
-    return e0.elapsed_time(e1) / steps
-
-
-# ----------------------------------------------------------------------------------------------
 # our arm
 # ----------------------------------------------------------------------------------------------
 def run_ours(args):
@@ -210,72 +171,17 @@ def run_ours(args):
     unit = list(multi.shard_units(world, rank, world))[0]
     wl.seed = wl.seed + 1000 * unit
 
-    gate_note = None
-    if args.kernel == "auto":
-        # rank 0 decides; the other ranks read its decision after the barrier
-        flag = os.path.join("/tmp", "ddsp_ring_gate_%s" % os.environ.get("MASTER_PORT", str(os.getpid())))
-        if rank == 0:
-            ok, gate_note = ring_gate()
-            with open(flag, "w") as f:
-                f.write("1" if ok else "0")
-        multi.barrier()
-        if open(flag).read().strip() == "1":
-            os.environ["DDSP_ENABLE_RING"] = "1"
-        multi.barrier()
-        if rank == 0:
-            os.remove(flag)
     plan = binding.plan_for(wl)
     in_pitch = synth.round_up(wl.nsamp, 128)
     out_pitch = synth.round_up(plan.nsamp_out, 32)
     plan.set_pitch(in_pitch, out_pitch)
-    plan.set_kernel({"auto": 0, "direct": 1, "tiled": 2, "ring": 3}[args.kernel])
+    plan.set_kernel({"auto": 0, "direct": 1, "tiled": 2}[args.kernel])
     x = synth.make_input(wl, dev, pitch=in_pitch, native_delays=library_native_delays(wl),
                          nsamp_out=plan.nsamp_out)
     out = torch.empty((plan.ndm, out_pitch), dtype=torch.int32 if wl.dtype == "u8" else torch.float32,
                       device=dev)
     stream = torch.cuda.current_stream(dev)
     adds = adds_per_execute(plan)
-    if args.kernel == "auto" and os.environ.get("DDSP_ENABLE_RING") == "1":
-        # both tiled kernels are verified here: run the faster one (measured on this workload)
-        t_ring = time_kernel(plan, x, out, stream, binding.DDSP_KERNEL_RING)
-        t_tiled = time_kernel(plan, x, out, stream, binding.DDSP_KERNEL_TILED)
-        pick = binding.DDSP_KERNEL_RING if t_ring is not None and (t_tiled is None or t_ring <= t_tiled) else \
-            (binding.DDSP_KERNEL_TILED if t_tiled is not None else binding.DDSP_KERNEL_AUTO)
-        plan.set_kernel(pick)
-        note = "; ms per execute: ring %s, tiled %s" % ("%.1f" % t_ring if t_ring else "n/a",
-                                                        "%.1f" % t_tiled if t_tiled else "n/a")
-        if pick == binding.DDSP_KERNEL_RING and wl.dtype == "u8" and wl.downsample == 1 and \
-                "DDSP_RING_VARIANT" not in os.environ:
-            # the compiled instantiations of the ring kernel differ in pipe balance and words per thread:
-            # time each on this workload, accept one only if its output equals the reference bit for bit
-            plan.execute(x, out, stream)
-            torch.cuda.synchronize(dev)
-            ref, out2 = out.clone(), torch.empty_like(out)
-            best_v, best_t = 0, t_ring
-            for v in (1, 2, 3, 4):
-                os.environ["DDSP_RING_VARIANT"] = str(v)
-                try:
-                    with binding.plan_for(wl) as p2:
-                        p2.set_pitch(in_pitch, out_pitch)
-                        t = time_kernel(p2, x, out2, stream, binding.DDSP_KERNEL_RING)
-                        same = t is not None and bool(torch.equal(out2[:, :plan.nsamp_out], ref[:, :plan.nsamp_out]))
-                except binding.DdspError:
-                    t, same = None, False
-                note += ", variant %d %s" % (v, ("%.1f" % t if same else "rejected") if t else "n/a")
-                if t is not None and same and t < best_t:
-                    best_v, best_t = v, t
-            del ref, out2
-            os.environ.pop("DDSP_RING_VARIANT", None)
-            if best_v:
-                os.environ["DDSP_RING_VARIANT"] = str(best_v)
-                plan.destroy()
-                plan = binding.plan_for(wl)
-                plan.set_pitch(in_pitch, out_pitch)
-                plan.set_kernel(binding.DDSP_KERNEL_RING)
-            note += "; running variant %d" % best_v
-        if gate_note is not None:
-            gate_note += note
-
     for _ in range(max(args.warmup, 0)):
         plan.execute(x, out, stream)
     torch.cuda.synchronize(dev)
@@ -327,8 +233,7 @@ def run_ours(args):
                        "nchan": wl.nchan, "nchan_unmasked": plan.nchan_unmasked, "ndm": plan.ndm,
                        "nsamp": wl.nsamp, "nsamp_out": plan.nsamp_out, "tsamp_s": wl.tsamp,
                        "downsample": wl.downsample, "in_dtype": wl.dtype,
-                       "kernel": {1: "direct", 2: "tiled", 3: "ring"}[plan.kernel],
-                       "ring_gate": gate_note,
+                       "kernel": {1: "direct", 2: "tiled"}[plan.kernel],
                        "units": "one observation per GPU", "parallelism": "dp%d" % world,
                        "l2": "inputs (%.2f GB) larger than L2; no flush" % (x.numel() * x.element_size() / 1e9)},
             "x_realtime": plan.nsamp_out * wl.tsamp * wl.downsample / (t_max / args.steps),
@@ -376,17 +281,7 @@ def measure_e2e(plan, wl, x, out, in_pitch, out_pitch, adds, steps, multi):
     xh = torch.empty(x.shape, dtype=x.dtype, pin_memory=True)
     xh.copy_(x)
     oh = torch.empty(out.shape, dtype=out.dtype, pin_memory=True)
-    from paper_2511_02328_b200 import binding
     call, how = plan.execute_host, "ddsp_execute_host (copy in, kernel, copy out in sequence)"
-    if plan.kernel == binding.DDSP_KERNEL_RING:
-        # the ring kernels can run on a range of time tiles: overlap copy-in, kernel and copy-out
-        try:
-            plan.execute_host_pipelined(xh, oh, nchunks=16)
-            if torch.equal(oh[:, :plan.nsamp_out], out[:, :plan.nsamp_out].cpu()):
-                call = lambda a, b: plan.execute_host_pipelined(a, b, nchunks=16)
-                how = "ddsp_execute_host_pipelined (16 pieces, copies and kernels overlapped)"
-        except binding.DdspError:
-            pass
     call(xh, oh)                                   # warm-up: allocates the staging buffers
     torch.cuda.synchronize()
     multi.barrier()

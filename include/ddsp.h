@@ -57,10 +57,7 @@ enum {
 enum {
     DDSP_KERNEL_AUTO = 0,
     DDSP_KERNEL_DIRECT = 1, /* one thread per output element, reads global memory directly (any plan) */
-    DDSP_KERNEL_TILED = 2,  /* shared-memory tiled kernel, rows staged through registers (first version) */
-    DDSP_KERNEL_RING = 3    /* shared-memory tiled kernel, rows staged by the copy engine into an mbarrier ring
-                               (DESIGN.md section 6); needs a 16-byte aligned input base pointer; uint8 with ds > 1 also
-                               a row pitch that is a multiple of 16; float32 only with ds = 1 */
+    DDSP_KERNEL_TILED = 2   /* shared-memory tiled kernel, rows staged through registers (uint8, ds = 1) */
 };
 
 /* Create a plan (the delay table is precomputed once, in double).
@@ -103,37 +100,6 @@ DDSP_API int ddsp_execute(const ddsp_plan* plan, const void* d_in, void* d_out, 
  * cuda_stream, and synchronises that stream before returning.  h_in: nchan rows of in_pitch elements;
  * h_out: ndm rows of out_pitch elements.  Not re-entrant for one plan (the staging buffers are shared). */
 DDSP_API int ddsp_execute_host(ddsp_plan* plan, const void* h_in, void* h_out, void* cuda_stream);
-
-/* ddsp_execute_host with the three phases overlapped (the paper names the copies, not the kernel, as its
- * bottleneck and leaves their overlap undone): the output columns are cut into
- * nchunks pieces (multiples of 2048 samples); piece j needs input columns < (end_j + d_max) * ds only, so
- * the copy of the input for piece j+1, the kernel of piece j and the copy of piece j-1's result run at the
- * same time on three internal streams.  Same buffers, layout and result as ddsp_execute_host; synchronises
- * cuda_stream first and returns when everything is done.  Pinned host memory is needed for real overlap.
- * DDSP_ERR_UNSUPPORTED unless the plan runs a ring kernel (DDSP_KERNEL_RING: the only kernels that can be
- * launched on a range of time tiles). */
-DDSP_API int ddsp_execute_host_pipelined(ddsp_plan* plan, const void* h_in, void* h_out, void* cuda_stream,
-                                         int nchunks);
-
-/* Introspection of the ring kernel's plan-time tables (tile geometry; DESIGN.md section
- * 6), so that the host logic can be tested without a GPU.  DDSP_ERR_UNSUPPORTED if the ring kernel cannot
- * run this plan.  geom: host int32[10] = {rows per stage C, DM blocks, chunks, padded channel count,
- * row stride (bytes of one phase copy), stages, table words per chunk, stage bytes, shared memory bytes,
- * tile length T}.  meta: host int64[blocks * padded channels]: bits 0..47 byte offset of the staged row
- * window at tile 0, bits 48.. its length in 16-byte units.  tbl: host uint32[blocks * chunks * table
- * words]: per chunk C x 32 stage-relative byte offsets ((slot * 4 + phase) * row stride + word offset),
- * then C unit counts.  rows: host int32[blocks * 32]: output row of each DM-sorted trial, -1 = padding. */
-DDSP_API int ddsp_plan_ring_geometry(const ddsp_plan* plan, int32_t* geom);
-DDSP_API int ddsp_plan_ring_tables(const ddsp_plan* plan, int64_t* meta, uint32_t* tbl, int32_t* rows);
-/* The same for the ring kernels of float32 input (ds = 1) and of uint8 input with ds > 1 (ddsp_ringx.cu).
- * geom: host int32[14] = {kind (1: uint8 16-bit bins, 2: float32), rows per chunk C, DM blocks, chunks,
- * padded channel count, raw row stride (bytes), bins row stride (bytes of one phase copy; kind 1), table words
- * per chunk, raw slots, bin slots, shared memory bytes, tile length T, channels between flushes (kind 1), raw
- * slot bytes}.  meta as above (byte offsets).  tbl per chunk: C x 32 byte offsets (kind 2: slot * raw stride +
- * 4 q; kind 1: (slot * 2 + (q & 1)) * bins stride + (q >> 1) * 4), then C unit counts (kind 2: 16-byte units of
- * the window; kind 1: 8-bin units), then (kind 1) C raw byte indices of the window start within the row. */
-DDSP_API int ddsp_plan_ringx_geometry(const ddsp_plan* plan, int32_t* geom);
-DDSP_API int ddsp_plan_ringx_tables(const ddsp_plan* plan, int64_t* meta, uint32_t* tbl, int32_t* rows);
 
 DDSP_API int ddsp_plan_destroy(ddsp_plan* plan); /* NULL is allowed */
 

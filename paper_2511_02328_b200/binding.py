@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libddsp.so")
 
 DDSP_IN_U8, DDSP_IN_F32 = 0, 1
 DDSP_OK, DDSP_ERR_INVALID_ARG, DDSP_ERR_NO_OUTPUT, DDSP_ERR_UNSUPPORTED, DDSP_ERR_ALLOC, DDSP_ERR_CUDA = range(6)
-DDSP_KERNEL_AUTO, DDSP_KERNEL_DIRECT, DDSP_KERNEL_TILED, DDSP_KERNEL_RING = 0, 1, 2, 3
+DDSP_KERNEL_AUTO, DDSP_KERNEL_DIRECT, DDSP_KERNEL_TILED = 0, 1, 2
 
 # name -> (restype, argtypes); one entry per declaration in include/ddsp.h
 _i, _i64, _f64, _vp, _cp = ctypes.c_int, ctypes.c_int64, ctypes.c_double, ctypes.c_void_p, ctypes.c_char_p
@@ -31,11 +31,6 @@ SIGNATURES = {
     "ddsp_plan_get_delays": (_i, [_vp, _vp]),
     "ddsp_execute": (_i, [_vp, _vp, _vp, _vp]),
     "ddsp_execute_host": (_i, [_vp, _vp, _vp, _vp]),
-    "ddsp_execute_host_pipelined": (_i, [_vp, _vp, _vp, _vp, _i]),
-    "ddsp_plan_ring_geometry": (_i, [_vp, _vp]),
-    "ddsp_plan_ring_tables": (_i, [_vp, _vp, _vp, _vp]),
-    "ddsp_plan_ringx_geometry": (_i, [_vp, _vp]),
-    "ddsp_plan_ringx_tables": (_i, [_vp, _vp, _vp, _vp]),
     "ddsp_plan_destroy": (_i, [_vp]),
     "ddsp_strerror": (_cp, [_i]),
     "ddsp_last_cuda_error": (_i, [_vp]),
@@ -120,40 +115,6 @@ class Plan:
         _check(lib().ddsp_plan_get_delays(self._h, out.ctypes.data), "ddsp_plan_get_delays", self._h)
         return out
 
-    def ring_geometry(self):
-        """ddsp_plan_ring_geometry as a dict (raises DdspError(UNSUPPORTED) if the ring kernel cannot run)."""
-        g = np.zeros(10, dtype=np.int32)
-        _check(lib().ddsp_plan_ring_geometry(self._h, g.ctypes.data), "ddsp_plan_ring_geometry", self._h)
-        names = ("c_rows", "nblk", "nchunk", "nch_pad", "row_stride", "nstage", "tblw", "stage_bytes",
-                 "smem_bytes", "tile_t")
-        return dict(zip(names, (int(v) for v in g)))
-
-    def ring_tables(self):
-        """ddsp_plan_ring_tables: (meta int64[nblk, nch_pad], tbl uint32[nblk, nchunk, tblw], rows int32[nblk, 32])."""
-        g = self.ring_geometry()
-        meta = np.zeros((g["nblk"], g["nch_pad"]), dtype=np.int64)
-        tbl = np.zeros((g["nblk"], g["nchunk"], g["tblw"]), dtype=np.uint32)
-        rows = np.zeros((g["nblk"], 32), dtype=np.int32)
-        _check(lib().ddsp_plan_ring_tables(self._h, meta.ctypes.data, tbl.ctypes.data, rows.ctypes.data),
-               "ddsp_plan_ring_tables", self._h)
-        return meta, tbl, rows
-
-    def ringx_geometry(self):
-        g = np.zeros(14, dtype=np.int32)
-        _check(lib().ddsp_plan_ringx_geometry(self._h, g.ctypes.data), "ddsp_plan_ringx_geometry", self._h)
-        names = ("kind", "c_rows", "nblk", "nchunk", "nch_pad", "raw_stride", "bins_stride", "tblw", "nraw",
-                 "nbins", "smem_bytes", "tile_t", "flush_every", "raw_slot_bytes")
-        return dict(zip(names, (int(v) for v in g)))
-
-    def ringx_tables(self):
-        g = self.ringx_geometry()
-        meta = np.zeros((g["nblk"], g["nch_pad"]), dtype=np.int64)
-        tbl = np.zeros((g["nblk"], g["nchunk"], g["tblw"]), dtype=np.uint32)
-        rows = np.zeros((g["nblk"], 32), dtype=np.int32)
-        _check(lib().ddsp_plan_ringx_tables(self._h, meta.ctypes.data, tbl.ctypes.data, rows.ctypes.data),
-               "ddsp_plan_ringx_tables", self._h)
-        return meta, tbl, rows
-
     # -- setters --------------------------------------------------------------------------------
     def set_pitch(self, in_pitch_elems, out_pitch_elems):
         _check(lib().ddsp_plan_set_pitch(self._h, int(in_pitch_elems), int(out_pitch_elems)),
@@ -185,17 +146,6 @@ class Plan:
         s = torch.cuda.current_stream() if stream is None else stream
         _check(lib().ddsp_execute_host(self._h, _vp(xp), _vp(op), _vp(s.cuda_stream)),
                "ddsp_execute_host", self._h)
-        return out
-
-    def execute_host_pipelined(self, x, out, stream=None, nchunks=8):
-        """ddsp_execute_host_pipelined: copies and kernels overlapped over `nchunks` pieces of the output columns."""
-        import torch
-        self._check_buffers(x, out, cuda=False)
-        xp = x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data
-        op = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
-        s = torch.cuda.current_stream() if stream is None else stream
-        _check(lib().ddsp_execute_host_pipelined(self._h, _vp(xp), _vp(op), _vp(s.cuda_stream), int(nchunks)),
-               "ddsp_execute_host_pipelined", self._h)
         return out
 
     def _check_buffers(self, x, out, cuda):

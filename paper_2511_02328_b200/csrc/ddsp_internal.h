@@ -35,50 +35,6 @@ struct ddsp_tiled {
     int nch_pad = 0;              // nchan_unmasked rounded up to chunk_c
 };
 
-// Geometry of the ring kernel (ddsp_ring.cu) for one plan.
-struct ddsp_ring {
-    bool ok = false;       // the ring kernel can run this plan
-    int variant = 0;       // index into the compiled instantiations
-    int c_rows = 0;        // channel rows per stage
-    int nblk = 0;          // DM blocks of 32 sorted trials
-    int64_t ntile_t = 0;   // time tiles of 2048 output samples
-    int row_stride = 0;    // bytes of shared memory per phase copy of a row
-    int tblw = 0;          // 32-bit words of the per-chunk table (offsets, unit counts)
-    int stage_bytes = 0;   // bytes per stage (rows x 4 phase copies + table)
-    int nstage = 0;        // stages in the ring
-    int smem_bytes = 0;    // dynamic shared memory per CTA
-    int nchunk = 0, nch_pad = 0;
-    int64_t* d_meta = nullptr;    // [nblk][nch_pad] row-window byte offset at t0 = 0 | units << 48
-    uint32_t* d_tbl = nullptr;    // [nblk][nchunk][tblw]
-    int32_t* d_rows = nullptr;    // [nblk * 32] output row of each sorted trial (-1 = padding)
-    std::vector<int64_t> h_meta;  // host copies (tests of the plan-time geometry)
-    std::vector<uint32_t> h_tbl;
-    std::vector<int32_t> h_rows;
-};
-
-// Geometry of the ring kernels for float32 input and for uint8 input with ds > 1 (ddsp_ringx.cu).
-struct ddsp_ringx {
-    bool ok = false;
-    int kind = 0;          // 1: uint8, ds > 1 (16-bit bins); 2: float32, ds = 1
-    int variant = 0;
-    int c_rows = 0;        // channel rows per chunk
-    int nblk = 0;          // DM blocks of 32 sorted trials
-    int tile_t = 0;        // output samples per tile
-    int64_t ntile_t = 0;
-    int raw_stride = 0;    // bytes per staged raw row
-    int bins_stride = 0;   // kind 1: bytes per phase copy of the 16-bit bins of a row
-    int tblw = 0;          // 32-bit words of the per-chunk table
-    int raw_slot_bytes = 0, bins_slot_bytes = 0, nraw = 0, nbins = 0, smem_bytes = 0;
-    int nchunk = 0, nch_pad = 0;
-    int flush_every = 0;   // kind 1: channels between flushes of the 16-bit lanes
-    int64_t* d_meta = nullptr;
-    uint32_t* d_tbl = nullptr;
-    int32_t* d_rows = nullptr;
-    std::vector<int64_t> h_meta;
-    std::vector<uint32_t> h_tbl;
-    std::vector<int32_t> h_rows;
-};
-
 struct ddsp_plan {
     // problem
     int nchan = 0, ndm = 0, ds = 1, in_dtype = DDSP_IN_U8;
@@ -97,16 +53,12 @@ struct ddsp_plan {
     int32_t* d_delays = nullptr;     // [ndm][nchan]
     int32_t* d_chan_list = nullptr;  // [nchan_unmasked]
     ddsp_tiled tiled;
-    ddsp_ring ring;
-    ddsp_ringx ringx;
     int kernel_req = DDSP_KERNEL_AUTO;
     int kernel = DDSP_KERNEL_DIRECT;
     mutable int last_cuda = 0;
     // staging buffers of ddsp_execute_host
     void* d_stage_in = nullptr;
     void* d_stage_out = nullptr;
-    // streams of ddsp_execute_host_pipelined (created on first use)
-    cudaStream_t hs_in = nullptr, hs_k = nullptr, hs_out = nullptr;
 };
 
 // ddsp_direct.cu
@@ -120,20 +72,3 @@ void ddsp_tiled_free(ddsp_plan* p);
 // true if this execute call meets the tiled kernel's alignment needs (16-byte base and row pitch)
 bool ddsp_tiled_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);
 cudaError_t ddsp_launch_tiled(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);
-
-// ddsp_ring.cu
-int ddsp_ring_plan(ddsp_plan* p);
-int ddsp_ring_set_pitch(ddsp_plan* p);    // rebuilds the pitch-dependent tables
-void ddsp_ring_free(ddsp_plan* p);
-bool ddsp_ring_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);   // 16-byte aligned input base
-// tile0 / ntile: range of time tiles (of the kernel's tile length) to compute; ntile < 0 = all from tile0 on
-cudaError_t ddsp_launch_ring(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s, int64_t tile0 = 0,
-                             int64_t ntile = -1);
-
-// ddsp_ringx.cu (same entry points as the ring kernel, for float32 and for uint8 with ds > 1)
-int ddsp_ringx_plan(ddsp_plan* p);
-int ddsp_ringx_set_pitch(ddsp_plan* p);
-void ddsp_ringx_free(ddsp_plan* p);
-bool ddsp_ringx_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);
-cudaError_t ddsp_launch_ringx(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s, int64_t tile0 = 0,
-                              int64_t ntile = -1);

@@ -27,7 +27,7 @@ size_t elem_size_in(const ddsp_plan* p) { return p->in_dtype == DDSP_IN_U8 ? 1 :
 
 void resolve_kernel(ddsp_plan* p) {
     if (p->kernel_req == DDSP_KERNEL_AUTO)
-        p->kernel = (p->ring.ok || p->ringx.ok) ? DDSP_KERNEL_RING : p->tiled.ok ? DDSP_KERNEL_TILED : DDSP_KERNEL_DIRECT;
+        p->kernel = p->tiled.ok ? DDSP_KERNEL_TILED : DDSP_KERNEL_DIRECT;
     else
         p->kernel = p->kernel_req;
 }
@@ -152,8 +152,6 @@ int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, 
         }
     }
     rc = ddsp_tiled_plan(p);
-    if (rc == DDSP_OK) rc = ddsp_ring_plan(p);
-    if (rc == DDSP_OK) rc = ddsp_ringx_plan(p);
     if (rc != DDSP_OK) { ddsp_plan_destroy(p); return rc; }
     resolve_kernel(p);
     *plan = p;
@@ -167,19 +165,15 @@ int ddsp_plan_set_pitch(ddsp_plan* p, int64_t in_pitch, int64_t out_pitch) {
     if (p->d_stage_in) { cudaFree(p->d_stage_in); p->d_stage_in = nullptr; }
     if (p->d_stage_out) { cudaFree(p->d_stage_out); p->d_stage_out = nullptr; }
     int rc = ddsp_tiled_set_pitch(p);
-    if (rc == DDSP_OK) rc = ddsp_ring_set_pitch(p);
-    if (rc == DDSP_OK) rc = ddsp_ringx_set_pitch(p);
     resolve_kernel(p);     // a pitch can disable a kernel that AUTO had chosen (16-byte row alignment)
     return rc;
 }
 
 int ddsp_plan_set_kernel(ddsp_plan* p, int kernel) {
     if (!p) return DDSP_ERR_INVALID_ARG;
-    if (kernel != DDSP_KERNEL_AUTO && kernel != DDSP_KERNEL_DIRECT && kernel != DDSP_KERNEL_TILED &&
-        kernel != DDSP_KERNEL_RING)
+    if (kernel != DDSP_KERNEL_AUTO && kernel != DDSP_KERNEL_DIRECT && kernel != DDSP_KERNEL_TILED)
         return DDSP_ERR_INVALID_ARG;
     if (kernel == DDSP_KERNEL_TILED && !p->tiled.ok) return DDSP_ERR_UNSUPPORTED;
-    if (kernel == DDSP_KERNEL_RING && !p->ring.ok && !p->ringx.ok) return DDSP_ERR_UNSUPPORTED;
     p->kernel_req = kernel;
     resolve_kernel(p);
     return DDSP_OK;
@@ -203,14 +197,7 @@ int ddsp_execute(const ddsp_plan* p, const void* d_in, void* d_out, void* cuda_s
     if (p->device < 0) return DDSP_ERR_CUDA;  // host-only plan: no device, no fallback
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e;
-    if (p->kernel == DDSP_KERNEL_RING) {
-        if (ddsp_ring_can_run(p, d_in, d_out)) e = ddsp_launch_ring(p, d_in, d_out, s);
-        else if (ddsp_ringx_can_run(p, d_in, d_out)) e = ddsp_launch_ringx(p, d_in, d_out, s);
-        else if (p->kernel_req == DDSP_KERNEL_RING) return DDSP_ERR_UNSUPPORTED;
-        // unaligned input base: correct through the register-staged or the direct kernel
-        else if (ddsp_tiled_can_run(p, d_in, d_out)) e = ddsp_launch_tiled(p, d_in, d_out, s);
-        else e = ddsp_launch_direct(p, d_in, d_out, s);
-    } else if (p->kernel == DDSP_KERNEL_TILED && !ddsp_tiled_can_run(p, d_in, d_out)) {
+    if (p->kernel == DDSP_KERNEL_TILED && !ddsp_tiled_can_run(p, d_in, d_out)) {
         // unaligned buffers: correct through the direct kernel unless the tiled one was forced
         if (p->kernel_req == DDSP_KERNEL_TILED) return DDSP_ERR_UNSUPPORTED;
         e = ddsp_launch_direct(p, d_in, d_out, s);
@@ -242,76 +229,13 @@ int ddsp_execute_host(ddsp_plan* p, const void* h_in, void* h_out, void* cuda_st
     return note_cuda(p, e);
 }
 
-int ddsp_execute_host_pipelined(ddsp_plan* p, const void* h_in, void* h_out, void* cuda_stream, int nchunks) {
-    if (!p || !h_in || !h_out || nchunks < 1) return DDSP_ERR_INVALID_ARG;
-    if (p->device < 0) return DDSP_ERR_CUDA;
-    // the ring kernels can be launched on a range of time tiles; the others cannot
-    if (p->kernel != DDSP_KERNEL_RING || (!p->ring.ok && !p->ringx.ok)) return DDSP_ERR_UNSUPPORTED;
-    const size_t esize = elem_size_in(p);
-    const size_t in_bytes = (size_t)p->nchan * (size_t)p->in_pitch * esize;
-    const size_t out_bytes = (size_t)p->ndm * (size_t)p->out_pitch * 4;
-    cudaError_t e = cudaSuccess;
-    if (!p->d_stage_in) e = cudaMalloc(&p->d_stage_in, in_bytes);
-    if (e == cudaSuccess && !p->d_stage_out) e = cudaMalloc(&p->d_stage_out, out_bytes);
-    if (e == cudaSuccess && !p->hs_in) e = cudaStreamCreateWithFlags(&p->hs_in, cudaStreamNonBlocking);
-    if (e == cudaSuccess && !p->hs_k) e = cudaStreamCreateWithFlags(&p->hs_k, cudaStreamNonBlocking);
-    if (e == cudaSuccess && !p->hs_out) e = cudaStreamCreateWithFlags(&p->hs_out, cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)cuda_stream);   // work queued before this call
-    if (e != cudaSuccess) return note_cuda(p, e);
-
-    const int64_t tile_t = p->ring.ok ? 2048 : p->ringx.tile_t;      // 1024 or 2048: chunks are multiples of 2048
-    const int64_t nout = p->nsamp_out;
-    int64_t chunk_cols = (nout + nchunks - 1) / nchunks;
-    chunk_cols = (chunk_cols + 2047) / 2048 * 2048;
-    const size_t in_pitch_b = (size_t)p->in_pitch * esize, out_pitch_b = (size_t)p->out_pitch * 4;
-    std::vector<cudaEvent_t> events;
-    int64_t in_done = 0;      // native input columns [0, in_done) are on the device (or on their way, in order)
-    for (int64_t a = 0; a < nout && e == cudaSuccess; a += chunk_cols) {
-        const int64_t b = std::min(a + chunk_cols, nout);
-        // outputs [a, b) read downsampled samples < b + d_max, i.e. native columns < (b + d_max) * ds
-        const int64_t need = std::min<int64_t>(p->nsamp, (b + p->dmax) * p->ds);
-        cudaEvent_t ev_in = nullptr, ev_k = nullptr;
-        e = cudaEventCreateWithFlags(&ev_in, cudaEventDisableTiming);
-        if (e == cudaSuccess) { events.push_back(ev_in); e = cudaEventCreateWithFlags(&ev_k, cudaEventDisableTiming); }
-        if (e == cudaSuccess) events.push_back(ev_k);
-        if (e == cudaSuccess && need > in_done) {
-            e = cudaMemcpy2DAsync((char*)p->d_stage_in + (size_t)in_done * esize, in_pitch_b,
-                                  (const char*)h_in + (size_t)in_done * esize, in_pitch_b,
-                                  (size_t)(need - in_done) * esize, (size_t)p->nchan, cudaMemcpyHostToDevice, p->hs_in);
-            in_done = need;
-        }
-        if (e == cudaSuccess) e = cudaEventRecord(ev_in, p->hs_in);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->hs_k, ev_in, 0);
-        if (e == cudaSuccess) {
-            const int64_t tile0 = a / tile_t, ntile = (b - a + tile_t - 1) / tile_t;
-            e = p->ring.ok ? ddsp_launch_ring(p, p->d_stage_in, p->d_stage_out, p->hs_k, tile0, ntile)
-                           : ddsp_launch_ringx(p, p->d_stage_in, p->d_stage_out, p->hs_k, tile0, ntile);
-        }
-        if (e == cudaSuccess) e = cudaEventRecord(ev_k, p->hs_k);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->hs_out, ev_k, 0);
-        if (e == cudaSuccess)
-            e = cudaMemcpy2DAsync((char*)h_out + (size_t)a * 4, out_pitch_b, (const char*)p->d_stage_out + (size_t)a * 4,
-                                  out_pitch_b, (size_t)(b - a) * 4, (size_t)p->ndm, cudaMemcpyDeviceToHost, p->hs_out);
-    }
-    // drain everything that was enqueued, also after an error
-    cudaError_t e1 = cudaStreamSynchronize(p->hs_in), e2 = cudaStreamSynchronize(p->hs_k), e3 = cudaStreamSynchronize(p->hs_out);
-    for (cudaEvent_t ev : events) cudaEventDestroy(ev);
-    if (e == cudaSuccess) e = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
-    return note_cuda(p, e);
-}
-
 int ddsp_plan_destroy(ddsp_plan* p) {
     if (!p) return DDSP_OK;
     ddsp_tiled_free(p);
-    ddsp_ring_free(p);
-    ddsp_ringx_free(p);
     if (p->d_delays) cudaFree(p->d_delays);
     if (p->d_chan_list) cudaFree(p->d_chan_list);
     if (p->d_stage_in) cudaFree(p->d_stage_in);
     if (p->d_stage_out) cudaFree(p->d_stage_out);
-    if (p->hs_in) cudaStreamDestroy(p->hs_in);
-    if (p->hs_k) cudaStreamDestroy(p->hs_k);
-    if (p->hs_out) cudaStreamDestroy(p->hs_out);
     delete p;
     return DDSP_OK;
 }

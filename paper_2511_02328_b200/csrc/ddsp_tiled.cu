@@ -38,17 +38,6 @@ constexpr int kTileT = kSlabs * kWT * 128;   // 2048 output samples per CTA (uin
 constexpr int kFlushEvery = 256;       // channels between flushes of the 16-bit lanes
 constexpr int kUnitsPerRowMax = 256;   // 16-byte units of a row window that the staging threads can cover
 
-// accumulation variants of the uint8 hot loop
-constexpr int kAccHybrid = 0;   // even lanes: LOP3 + IADD3 (two rows per add); odd lanes: PRMT + IMAD
-constexpr int kAccWide = 1;     // even lanes: LOP3 + IADD3; whole word: one IMAD.WIDE into a 64-bit sum
-constexpr int kAccAllFma = 2;   // both lanes: extract on the ALU pipe, every add an IMAD
-constexpr int kAccAllAlu = 3;   // both lanes: extract + IADD3 (two rows per add), nothing on the FMA pipe
-// "full word" variants: accE accumulates the WHOLE word (mod 2^32), accO the odd bytes (PRMT).  At flush
-// accE - (accO << 8) = B0 + 2^16 B2 exactly (mod 2^32), so the even bytes never need extracting.
-constexpr int kAccFullP = 4;    // whole word: IADD3 (two rows per add);  odd bytes: PRMT + IMAD
-constexpr int kAccFullQ = 5;    // whole word: IMAD;                      odd bytes: PRMT + IMAD
-constexpr int kAccFullR = 6;    // whole word: IADD3;                     odd bytes: PRMT + IADD3
-
 struct TiledArgs {
     const uint8_t* in;
     uint32_t* out;
@@ -58,8 +47,6 @@ struct TiledArgs {
     const int32_t* rows;      // [nblk * bdm] output row of each sorted trial, -1 = padding
     int64_t out_pitch, nsamp_out, in_bytes;
     int nlist, nch_pad, nblk, chunk_shift, nchunk, row_stride, out_vec, in_vec;
-    int debug_nostage;        // tuning only: skip staging after the first chunk (wrong results)
-    uint32_t one;             // 1: multiplier that routes an add through the FMA pipe (IMAD / IMAD.WIDE)
 };
 
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
@@ -70,20 +57,13 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
 __device__ __forceinline__ void lds128(uint32_t addr, uint32_t* v) {
     asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(addr));
 }
-// acc += v on the FMA pipe (IMAD): the ALU pipe (LOP3/PRMT/IADD3, 64 lanes/clk/SM) is the busier one
-__device__ __forceinline__ void add_fma_pipe(uint32_t& acc, uint32_t v, uint32_t one) {
-    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(acc) : "r"(v), "r"(one));
-}
-__device__ __forceinline__ void add_wide(uint64_t& acc, uint32_t v, uint32_t one) {
-    asm("mad.wide.u32 %0, %1, %2, %0;" : "+l"(acc) : "r"(v), "r"(one));
-}
-
 // ------------------------------------------------------------------------------------------------
 // uint8, ds = 1
 // ------------------------------------------------------------------------------------------------
-// BDM_T trials per thread, GROUPS trial groups (BDM = GROUPS * BDM_T trials per CTA, 128 * GROUPS
-// threads), MODE = accumulation variant
-template <int BDM_T, int GROUPS, int MODE>
+// BDM_T trials per thread, GROUPS trial groups (BDM = GROUPS * BDM_T trials per CTA, 128 * GROUPS threads).
+// accE accumulates the WHOLE word (mod 2^32), accO the odd bytes (PRMT) in two 16-bit lanes.  At flush
+// accE - (accO << 8) = B0 + 2^16 B2 exactly (mod 2^32), so the even bytes never need extracting.
+template <int BDM_T, int GROUPS>
 __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const TiledArgs a) {
     constexpr int BDM = GROUPS * BDM_T;
     constexpr int kThreads = 32 * kSlabs * GROUPS;
@@ -107,18 +87,13 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
     const uint32_t* __restrict__ off_b = a.off + (size_t)blk * a.nch_pad * BDM;
 
     // packed accumulators of each owned word (4 consecutive samples s0..s3):
-    //   accE = (s0, s2) in 16-bit lanes; accO = (s1, s3) [hybrid] / accW = 64-bit sum of whole words [wide]
+    //   accE = sum of whole words; accO = (s1, s3) in 16-bit lanes
     uint32_t accE[BDM_T][kWT];
-    uint32_t accO[MODE != kAccWide ? BDM_T : 1][kWT];
-    uint64_t accW[MODE == kAccWide ? BDM_T : 1][kWT];
+    uint32_t accO[BDM_T][kWT];
 #pragma unroll
     for (int k = 0; k < kWT; ++k) {
 #pragma unroll
-        for (int j = 0; j < BDM_T; ++j) accE[j][k] = 0;
-#pragma unroll
-        for (int j = 0; j < (MODE != kAccWide ? BDM_T : 1); ++j) accO[j][k] = 0;
-#pragma unroll
-        for (int j = 0; j < (MODE == kAccWide ? BDM_T : 1); ++j) accW[j][k] = 0;
+        for (int j = 0; j < BDM_T; ++j) { accE[j][k] = 0; accO[j][k] = 0; }
     }
 
     // Staging: 512 / chunk_c consecutive threads serve one row slot; a thread owns the 16-byte units
@@ -201,24 +176,16 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
             for (int k = 0; k < kWT; ++k) {
                 const int64_t t = t0 + slab * (kWT * 128) + k * 128 + lane * 4;
                 uint32_t e = 0, o = 0;
-                uint64_t ws = 0;
 #pragma unroll
                 for (int jj = 0; jj < BDM_T; ++jj)      // static register indexing under a rolled loop
                     if (jj == j) {
                         e = accE[jj][k]; accE[jj][k] = 0;
-                        if (MODE != kAccWide) { o = accO[jj][k]; accO[jj][k] = 0; }
-                        if (MODE == kAccWide) { ws = accW[jj][k]; accW[jj][k] = 0; }
+                        o = accO[jj][k]; accO[jj][k] = 0;
                     }
                 if (row < 0 || t >= a.nsamp_out) continue;
                 uint32_t* p = a.out + (size_t)row * (size_t)a.out_pitch + t;
-                if (MODE >= kAccFullP) e -= o << 8;     // whole-word sum -> even bytes (exact mod 2^32)
-                uint32_t v0 = e & 0xffffu, v2 = e >> 16, v1, v3;
-                if (MODE != kAccWide) {
-                    v1 = o & 0xffffu; v3 = o >> 16;
-                } else {   // sum(w) = B0 + 2^8 B1 + 2^16 B2 + 2^24 B3 and e = B0 + 2^16 B2
-                    const uint64_t r = ws - (uint64_t)e;
-                    v1 = (uint32_t)(r >> 8) & 0xffffu; v3 = (uint32_t)(r >> 24);
-                }
+                e -= o << 8;     // whole-word sum -> even bytes (exact mod 2^32)
+                uint32_t v0 = e & 0xffffu, v2 = e >> 16, v1 = o & 0xffffu, v3 = o >> 16;
                 if (a.out_vec && t + 3 < a.nsamp_out) {
                     if (!first_flush) {
                         const uint4 old = *reinterpret_cast<const uint4*>(p);
@@ -238,7 +205,6 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
 
     // byte offset of this thread's first word inside a phase copy (relative to the row window start)
     const uint32_t lane_off = (uint32_t)(slab * (kWT * 128) + lane * 4);
-    const uint32_t one = a.one;
 
     meta_cur = load_meta(0);
     meta_nxt = load_meta(1);
@@ -247,8 +213,8 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
     __syncthreads();
     int since_flush = 0;
     for (int chunk = 0; chunk < a.nchunk; ++chunk) {
-        const int stage = a.debug_nostage ? 0 : (chunk & 1);
-        const bool more = chunk + 1 < a.nchunk && !a.debug_nostage;
+        const int stage = chunk & 1;
+        const bool more = chunk + 1 < a.nchunk;
         meta_cur = meta_nxt;                     // arrived during the previous chunk
         meta_nxt = load_meta(chunk + 2);
         if (more) prefetch(chunk + 1, meta_cur);
@@ -274,26 +240,8 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
 #pragma unroll
                 for (int k = 0; k < kWT; ++k) {
                     const uint32_t w0 = lds32(a0 + k * 128), w1 = lds32(a1 + k * 128);
-                    if (MODE == kAccAllFma) {
-                        add_fma_pipe(accE[j][k], w0 & 0x00ff00ffu, one);
-                        add_fma_pipe(accE[j][k], w1 & 0x00ff00ffu, one);
-                    } else if (MODE == kAccFullP || MODE == kAccFullR) {
-                        accE[j][k] = accE[j][k] + w0 + w1;
-                    } else if (MODE == kAccFullQ) {
-                        add_fma_pipe(accE[j][k], w0, one);
-                        add_fma_pipe(accE[j][k], w1, one);
-                    } else {
-                        accE[j][k] = accE[j][k] + (w0 & 0x00ff00ffu) + (w1 & 0x00ff00ffu);   // IADD3 (ALU pipe)
-                    }
-                    if (MODE == kAccHybrid || MODE == kAccAllFma || MODE == kAccFullP || MODE == kAccFullQ) {
-                        add_fma_pipe(accO[j][k], __byte_perm(w0, 0, 0x4341), one);      // IMAD  (FMA pipe)
-                        add_fma_pipe(accO[j][k], __byte_perm(w1, 0, 0x4341), one);
-                    } else if (MODE == kAccAllAlu || MODE == kAccFullR) {
-                        accO[j][k] = accO[j][k] + __byte_perm(w0, 0, 0x4341) + __byte_perm(w1, 0, 0x4341);
-                    } else {
-                        add_wide(accW[j][k], w0, one);                                  // IMAD.WIDE
-                        add_wide(accW[j][k], w1, one);
-                    }
+                    accE[j][k] = accE[j][k] + w0 + w1;                                              // IADD3
+                    accO[j][k] = accO[j][k] + __byte_perm(w0, 0, 0x4341) + __byte_perm(w1, 0, 0x4341);    // 2 PRMT + IADD3
                 }
             }
         }
@@ -307,9 +255,8 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
 #pragma unroll
                 for (int k = 0; k < kWT; ++k) {
                     const uint32_t w0 = lds32(a0 + k * 128);
-                    accE[j][k] += (MODE >= kAccFullP) ? w0 : (w0 & 0x00ff00ffu);
-                    if (MODE != kAccWide) accO[j][k] += __byte_perm(w0, 0, 0x4341);
-                    else accW[j][k] += w0;
+                    accE[j][k] += w0;
+                    accO[j][k] += __byte_perm(w0, 0, 0x4341);
                 }
             }
         }
@@ -320,21 +267,9 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
 }
 
 typedef void (*TiledKernel)(const TiledArgs);
-struct Variant { int bdm_t; int groups; int mode; TiledKernel fn; };
+struct Variant { int bdm_t; int groups; TiledKernel fn; };
 const Variant kVariants[] = {
-    // order of preference (measured on config "fast", cropped to 600k samples: 17.3 / 17.3 / 16.4 / 16.0 /
-    // 14.5 / 14.3 / 13.8 / 12.1 / 11.1 Tadd/s)
-    {8, 4, kAccFullR, ddsp_tiled_u8_kernel<8, 4, kAccFullR>},     // 32 trials, 512 threads
-    {8, 4, kAccFullP, ddsp_tiled_u8_kernel<8, 4, kAccFullP>},
-    {8, 4, kAccFullQ, ddsp_tiled_u8_kernel<8, 4, kAccFullQ>},
-    {8, 4, kAccAllFma, ddsp_tiled_u8_kernel<8, 4, kAccAllFma>},
-    {8, 4, kAccHybrid, ddsp_tiled_u8_kernel<8, 4, kAccHybrid>},
-    {8, 4, kAccAllAlu, ddsp_tiled_u8_kernel<8, 4, kAccAllAlu>},
-    {4, 4, kAccHybrid, ddsp_tiled_u8_kernel<4, 4, kAccHybrid>},   // 16 trials, 512 threads
-    {4, 8, kAccHybrid, ddsp_tiled_u8_kernel<4, 8, kAccHybrid>},   // 32 trials, 1024 threads, <= 64 registers
-    {4, 4, kAccWide, ddsp_tiled_u8_kernel<4, 4, kAccWide>},
-    {4, 8, kAccFullR, ddsp_tiled_u8_kernel<4, 8, kAccFullR>},     // 32 trials, 1024 threads
-    {4, 8, kAccFullP, ddsp_tiled_u8_kernel<4, 8, kAccFullP>},
+    {8, 4, ddsp_tiled_u8_kernel<8, 4>},     // 32 trials, 512 threads
 };
 constexpr int kNumVariants = sizeof(kVariants) / sizeof(kVariants[0]);
 
@@ -456,14 +391,7 @@ int ddsp_tiled_plan(ddsp_plan* p) {
     g.ok = false;
     const int nlist = (int)p->chan_list.size();
     if (p->in_dtype != DDSP_IN_U8 || p->ds != 1 || nlist < 1) return DDSP_OK;   // other paths: direct kernel
-    // Variants in order of preference; a forced variant (DDSP_TILED_VARIANT, tuning only) comes first.
-    int forced = -1;
-    if (const char* ev = getenv("DDSP_TILED_VARIANT")) forced = atoi(ev);
-    for (int k = -1; k < kNumVariants && !g.ok; ++k) {
-        const int v = k < 0 ? forced : k;
-        if (v < 0 || v >= kNumVariants) continue;
-        g.ok = tiled_geometry(p, v, g);
-    }
+    for (int v = 0; v < kNumVariants && !g.ok; ++v) g.ok = tiled_geometry(p, v, g);
     if (!g.ok) return DDSP_OK;
     return tiled_build_tables(p);
 }
@@ -503,8 +431,7 @@ cudaError_t ddsp_launch_tiled(const ddsp_plan* p, const void* d_in, void* d_out,
     a.in = (const uint8_t*)d_in;
     a.out = (uint32_t*)d_out;
     a.meta = g.d_meta; a.off = g.d_off; a.rows = g.d_rows;
-    a.out_pitch = p->out_pitch; a.nsamp_out = p->nsamp_out; a.one = 1u;
-    a.debug_nostage = getenv("DDSP_DEBUG_NOSTAGE") ? 1 : 0;
+    a.out_pitch = p->out_pitch; a.nsamp_out = p->nsamp_out;
     a.in_bytes = (int64_t)p->nchan * p->in_pitch;
     a.nlist = (int)p->chan_list.size(); a.nch_pad = g.nch_pad; a.nblk = g.nblk;
     a.chunk_shift = g.chunk_shift; a.nchunk = g.nchunk; a.row_stride = g.row_stride;

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_2511_02328_b200", "csrc")
 BUILD = os.path.join(HERE, "build")
-PRODUCT = ["ddsp_plan.cpp", "ddsp_ring.cu", "ddsp_ringx.cu", "ddsp_tiled.cu", "ddsp_direct.cu"]
+PRODUCT = ["ddsp_plan.cpp", "ddsp_tiled.cu", "ddsp_direct.cu"]
 LIB = os.path.join(BUILD, "libddsp_emu.so")
 TSAN_EXE = os.path.join(BUILD, "emu_tsan")
 

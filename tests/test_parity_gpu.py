@@ -15,8 +15,8 @@ from _util import (assert_f32_close, assert_u32_equal, crop, make_input, oracle_
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [binding.DDSP_KERNEL_DIRECT, binding.DDSP_KERNEL_TILED, binding.DDSP_KERNEL_RING]
-KNAME = {binding.DDSP_KERNEL_DIRECT: "direct", binding.DDSP_KERNEL_TILED: "tiled", binding.DDSP_KERNEL_RING: "ring"}
+KERNELS = [binding.DDSP_KERNEL_DIRECT, binding.DDSP_KERNEL_TILED]
+KNAME = {binding.DDSP_KERNEL_DIRECT: "direct", binding.DDSP_KERNEL_TILED: "tiled"}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -234,20 +234,6 @@ def test_execute_host_matches_device(oracle):
         oh = torch.empty((plan.ndm, plan.out_pitch), dtype=torch.int32).pin_memory()
         plan.execute_host(xh, oh)
         assert np.array_equal(oh.numpy().view(np.uint32), dev)
-
-
-@pytest.mark.parametrize("nchunks", [1, 3, 8])
-def test_execute_host_pipelined_ring(oracle, nchunks):
-    """Overlapped host-buffer execute (ring kernels only): same result as the oracle, whatever the piece count."""
-    wl = _small(nsamp=9000)
-    x = make_input(oracle, wl, "cuda")
-    with binding.plan_for(wl) as plan:
-        _set_kernel(plan, binding.DDSP_KERNEL_RING)
-        xh = x.cpu().pin_memory()
-        oh = torch.full((plan.ndm, plan.out_pitch), -5, dtype=torch.int32).pin_memory()
-        plan.execute_host_pipelined(xh, oh, nchunks=nchunks)
-        want, _, _ = oracle.dedisperse(xh.numpy(), wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list)
-        assert_u32_equal(oh.numpy().view(np.uint32)[:, :plan.nsamp_out], want, "pipelined")
 
 
 def test_two_streams_concurrent(oracle):
