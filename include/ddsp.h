@@ -22,8 +22,11 @@
  *     that was current when the plan was created;
  *   - the plan copies dm_list and chan_mask at create; it owns its device tables and frees them in
  *     ddsp_plan_destroy; input/output buffers are always caller-owned;
- *   - a plan is immutable after create / set_pitch / set_kernel; concurrent ddsp_execute calls on
- *     different streams with different buffers are legal.
+ *   - ddsp_execute never changes the plan: after create / set_pitch / set_kernel, concurrent ddsp_execute
+ *     calls on different streams with different buffers are legal for kernels without a workspace, and
+ *     through ddsp_execute_ws (one workspace per concurrent call) for the others;
+ *   - ddsp_plan_set_pitch, ddsp_plan_set_kernel and ddsp_execute_host DO change the plan (tables, workspace,
+ *     staging buffers): they must not run concurrently with anything else on the same plan.
  */
 #ifndef DDSP_H
 #define DDSP_H
@@ -57,7 +60,9 @@ enum {
 enum {
     DDSP_KERNEL_AUTO = 0,
     DDSP_KERNEL_DIRECT = 1, /* one thread per output element, reads global memory directly (any plan) */
-    DDSP_KERNEL_TILED = 2   /* shared-memory tiled kernel, rows staged through registers (uint8, ds = 1) */
+    DDSP_KERNEL_TILED = 2,  /* shared-memory tiled kernel, rows staged through registers (uint8, ds = 1) */
+    DDSP_KERNEL_LANES = 3   /* segment-interleaved kernels: an interleave pass into a workspace,
+                               then a persistent kernel fed by the copy engine; uint8 (ds <= 64) and float32 */
 };
 
 /* Create a plan (the delay table is precomputed once, in double).
@@ -83,6 +88,14 @@ DDSP_API int64_t ddsp_plan_max_delay(const ddsp_plan* plan);      /* d_max on th
 DDSP_API int ddsp_plan_nchan_unmasked(const ddsp_plan* plan);     /* channels that enter the sum */
 DDSP_API int ddsp_plan_kernel(const ddsp_plan* plan);             /* the kernel ddsp_execute will launch (resolved AUTO) */
 DDSP_API int ddsp_plan_launches_per_execute(const ddsp_plan* plan); /* kernel launches one ddsp_execute enqueues */
+/* Bytes of device workspace one execute of the plan's kernel needs (0: none).  The plan owns one workspace of
+ * that size (allocated by ddsp_plan_create / ddsp_plan_set_kernel, never by ddsp_execute), which every
+ * ddsp_execute of the plan uses; ddsp_execute_ws takes the caller's instead. */
+DDSP_API int64_t ddsp_plan_workspace_bytes(const ddsp_plan* plan);
+/* Device-side status of the plan's kernels: *status = 0 ok, 1 a bounded barrier wait ran out (the kernel ended
+ * early instead of hanging; its output is invalid), 2 a plan table failed the kernel's own bounds check.
+ * Copies one word from the device (synchronises with the work in flight). */
+DDSP_API int ddsp_plan_device_status(ddsp_plan* plan, int* status);
 
 /* Copy the plan's delay table d(i,c), row-major [ndm][nchan] in dm_list order, to host memory. */
 DDSP_API int ddsp_plan_get_delays(const ddsp_plan* plan, int32_t* host_out);
@@ -95,9 +108,17 @@ DDSP_API int ddsp_plan_get_delays(const ddsp_plan* plan, int32_t* host_out);
  * asynchronous faults surface at the caller's next synchronisation. */
 DDSP_API int ddsp_execute(const ddsp_plan* plan, const void* d_in, void* d_out, void* cuda_stream);
 
+/* ddsp_execute with a caller-owned workspace: d_ws = device memory, 16-byte aligned, ws_bytes >=
+ * ddsp_plan_workspace_bytes(plan) (d_ws = NULL: the plan's own).  Executes of ONE plan that may overlap in
+ * time (different streams) must not share a workspace: give each its own through this call.  Kernels that
+ * need no workspace ignore it. */
+DDSP_API int ddsp_execute_ws(const ddsp_plan* plan, const void* d_in, void* d_out, void* d_ws, int64_t ws_bytes,
+                             void* cuda_stream);
+
 /* Same operation on HOST buffers (pinned memory recommended): copies h_in to a device staging buffer
- * owned by the plan (allocated on first use), runs ddsp_execute, copies the result to h_out, all on
- * cuda_stream, and synchronises that stream before returning.  h_in: nchan rows of in_pitch elements;
+ * owned by the plan (allocated on the first call after create / set_pitch, freed by set_pitch and destroy),
+ * runs ddsp_execute, copies the result to h_out, all on cuda_stream, and synchronises that stream before
+ * returning.  h_in: nchan rows of in_pitch elements;
  * h_out: ndm rows of out_pitch elements.  Not re-entrant for one plan (the staging buffers are shared). */
 DDSP_API int ddsp_execute_host(ddsp_plan* plan, const void* h_in, void* h_out, void* cuda_stream);
 

@@ -15,7 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libddsp.so")
 
 DDSP_IN_U8, DDSP_IN_F32 = 0, 1
 DDSP_OK, DDSP_ERR_INVALID_ARG, DDSP_ERR_NO_OUTPUT, DDSP_ERR_UNSUPPORTED, DDSP_ERR_ALLOC, DDSP_ERR_CUDA = range(6)
-DDSP_KERNEL_AUTO, DDSP_KERNEL_DIRECT, DDSP_KERNEL_TILED = 0, 1, 2
+DDSP_KERNEL_AUTO, DDSP_KERNEL_DIRECT, DDSP_KERNEL_TILED, DDSP_KERNEL_LANES = 0, 1, 2, 3
 
 # name -> (restype, argtypes); one entry per declaration in include/ddsp.h
 _i, _i64, _f64, _vp, _cp = ctypes.c_int, ctypes.c_int64, ctypes.c_double, ctypes.c_void_p, ctypes.c_char_p
@@ -28,8 +28,11 @@ SIGNATURES = {
     "ddsp_plan_nchan_unmasked": (_i, [_vp]),
     "ddsp_plan_kernel": (_i, [_vp]),
     "ddsp_plan_launches_per_execute": (_i, [_vp]),
+    "ddsp_plan_workspace_bytes": (_i64, [_vp]),
+    "ddsp_plan_device_status": (_i, [_vp, _vp]),
     "ddsp_plan_get_delays": (_i, [_vp, _vp]),
     "ddsp_execute": (_i, [_vp, _vp, _vp, _vp]),
+    "ddsp_execute_ws": (_i, [_vp, _vp, _vp, _vp, _i64, _vp]),
     "ddsp_execute_host": (_i, [_vp, _vp, _vp, _vp]),
     "ddsp_plan_destroy": (_i, [_vp]),
     "ddsp_strerror": (_cp, [_i]),
@@ -110,6 +113,16 @@ class Plan:
     def launches_per_execute(self):
         return int(lib().ddsp_plan_launches_per_execute(self._h))
 
+    @property
+    def workspace_bytes(self):
+        return int(lib().ddsp_plan_workspace_bytes(self._h))
+
+    def device_status(self):
+        """ddsp_plan_device_status: 0 ok, 1 bounded wait ran out, 2 table bounds check (synchronises)."""
+        st = ctypes.c_int(0)
+        _check(lib().ddsp_plan_device_status(self._h, ctypes.byref(st)), "ddsp_plan_device_status", self._h)
+        return int(st.value)
+
     def get_delays(self):
         out = np.empty((self.ndm, self.nchan), dtype=np.int32)
         _check(lib().ddsp_plan_get_delays(self._h, out.ctypes.data), "ddsp_plan_get_delays", self._h)
@@ -129,12 +142,18 @@ class Plan:
         """Raw form: device addresses as integers, cudaStream_t as integer."""
         _check(lib().ddsp_execute(self._h, _vp(d_in), _vp(d_out), _vp(cuda_stream)), "ddsp_execute", self._h)
 
-    def execute(self, x, out, stream=None):
-        """x, out: torch CUDA tensors shaped (nchan, in_pitch) and (ndm, out_pitch)."""
+    def execute(self, x, out, stream=None, workspace=None):
+        """x, out: torch CUDA tensors shaped (nchan, in_pitch) and (ndm, out_pitch); workspace: optional torch
+        CUDA uint8 tensor of at least workspace_bytes (ddsp_execute_ws), else the plan's own."""
         import torch
         self._check_buffers(x, out, cuda=True)
         s = torch.cuda.current_stream(x.device) if stream is None else stream
-        self.execute_ptr(x.data_ptr(), out.data_ptr(), s.cuda_stream)
+        if workspace is None:
+            self.execute_ptr(x.data_ptr(), out.data_ptr(), s.cuda_stream)
+        else:
+            _check(lib().ddsp_execute_ws(self._h, _vp(x.data_ptr()), _vp(out.data_ptr()), _vp(workspace.data_ptr()),
+                                         int(workspace.numel() * workspace.element_size()), _vp(s.cuda_stream)),
+                   "ddsp_execute_ws", self._h)
         return out
 
     def execute_host(self, x, out, stream=None):

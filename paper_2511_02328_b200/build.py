@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libddsp.so")
-SOURCES = ["ddsp_plan.cpp", "ddsp_direct.cu", "ddsp_tiled.cu"]
+SOURCES = ["ddsp_plan.cpp", "ddsp_direct.cu", "ddsp_tiled.cu", "ddsp_lanes.cu"]
 HEADERS = [os.path.join(CSRC, "ddsp_internal.h"), os.path.join(_ROOT, "include", "ddsp.h")]
 NVCC_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",

@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdint>
 #include <vector>
 
@@ -35,6 +36,28 @@ struct ddsp_tiled {
     int nch_pad = 0;              // nchan_unmasked rounded up to chunk_c
 };
 
+// Geometry of the lanes kernels (ddsp_lanes.cu) for one plan.
+enum { DDSP_LANES_U8 = 0, DDSP_LANES_U16 = 1, DDSP_LANES_F32 = 2 };
+struct ddsp_lanes {
+    bool ok = false;       // the lanes kernel can run this plan
+    int kind = 0;          // DDSP_LANES_U8 (uint8, ds = 1), _U16 (uint8, ds > 1: 16-bit bins), _F32
+    int nblk = 0;          // blocks of 16 DM-sorted trials
+    int nchunk = 0;        // chunks of 4 listed channels
+    int RS = 0;            // bytes of shared memory per staged row window (the longest window of the plan)
+    int NS = 0;            // ring stages
+    int stage_bytes = 0, smem_bytes = 0;
+    int flush_rows = 0;    // channels between flushes of the 16-bit lanes
+    size_t ws_bytes = 0;   // workspace (interleaved copy of the unmasked rows) for a full execute
+    int2* d_win = nullptr;        // [nblk][nchunk * 4] {first word of the row window relative to the tile, words}
+    uint32_t* d_off = nullptr;    // [nblk][nchunk][4 * 16] stage-relative byte offset of every (row, trial)
+    int32_t* d_rows = nullptr;    // [nblk * 16] output row of each sorted trial (-1 = padding)
+    int* d_status = nullptr;      // device status word (0 = ok) written by the kernels
+    uint8_t* d_ws = nullptr;      // the plan's own workspace
+    std::vector<int2> h_win;      // host copies (uploaded by ddsp_lanes_prepare; read by the table tests)
+    std::vector<uint32_t> h_off;
+    std::vector<int32_t> h_rows;
+};
+
 struct ddsp_plan {
     // problem
     int nchan = 0, ndm = 0, ds = 1, in_dtype = DDSP_IN_U8;
@@ -53,9 +76,10 @@ struct ddsp_plan {
     int32_t* d_delays = nullptr;     // [ndm][nchan]
     int32_t* d_chan_list = nullptr;  // [nchan_unmasked]
     ddsp_tiled tiled;
+    ddsp_lanes lanes;
     int kernel_req = DDSP_KERNEL_AUTO;
     int kernel = DDSP_KERNEL_DIRECT;
-    mutable int last_cuda = 0;
+    mutable std::atomic<int> last_cuda{0};   // written by concurrent executes
     // staging buffers of ddsp_execute_host
     void* d_stage_in = nullptr;
     void* d_stage_out = nullptr;
@@ -72,3 +96,13 @@ void ddsp_tiled_free(ddsp_plan* p);
 // true if this execute call meets the tiled kernel's alignment needs (16-byte base and row pitch)
 bool ddsp_tiled_can_run(const ddsp_plan* p, const void* d_in, const void* d_out);
 cudaError_t ddsp_launch_tiled(const ddsp_plan* p, const void* d_in, void* d_out, cudaStream_t s);
+
+// ddsp_lanes.cu
+int ddsp_lanes_plan(ddsp_plan* p);        // host geometry + tables (p->lanes.ok false = unsupported)
+int ddsp_lanes_prepare(ddsp_plan* p);     // device tables, status word, the plan's workspace (idempotent)
+void ddsp_lanes_free(ddsp_plan* p);
+// segment geometry of a run of nout output columns: tiles, columns per segment, words per interleaved row
+void ddsp_lanes_range(const ddsp_plan* p, int64_t nout, int64_t* NT, int64_t* Q, int64_t* M);
+// output columns [u_begin, u_begin + nout) (nout < 0: to the end); ws = NULL: the plan's workspace
+cudaError_t ddsp_launch_lanes(const ddsp_plan* p, const void* d_in, void* d_out, void* ws, cudaStream_t s,
+                              int64_t u_begin = 0, int64_t nout = -1);

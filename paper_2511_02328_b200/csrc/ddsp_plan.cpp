@@ -25,9 +25,16 @@ int note_cuda(const ddsp_plan* p, cudaError_t e) {
 
 size_t elem_size_in(const ddsp_plan* p) { return p->in_dtype == DDSP_IN_U8 ? 1 : 4; }
 
+// AUTO takes the lanes kernels only after they have passed their parity tests on a B200 (DESIGN.md section 8
+// records the log); until then they run on request (ddsp_plan_set_kernel) and AUTO stays with the kernels that
+// have a hardware history.  Flipped in code, by a commit that cites the log -- never by the environment.
+constexpr bool kAutoTakesLanes = false;
+
 void resolve_kernel(ddsp_plan* p) {
     if (p->kernel_req == DDSP_KERNEL_AUTO)
-        p->kernel = p->tiled.ok ? DDSP_KERNEL_TILED : DDSP_KERNEL_DIRECT;
+        p->kernel = (kAutoTakesLanes && p->lanes.ok) ? DDSP_KERNEL_LANES
+                    : p->tiled.ok                    ? DDSP_KERNEL_TILED
+                                                     : DDSP_KERNEL_DIRECT;
     else
         p->kernel = p->kernel_req;
 }
@@ -152,8 +159,12 @@ int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, 
         }
     }
     rc = ddsp_tiled_plan(p);
+    if (rc == DDSP_OK) rc = ddsp_lanes_plan(p);
+    if (rc == DDSP_OK) {
+        resolve_kernel(p);
+        if (p->kernel == DDSP_KERNEL_LANES) rc = ddsp_lanes_prepare(p);
+    }
     if (rc != DDSP_OK) { ddsp_plan_destroy(p); return rc; }
-    resolve_kernel(p);
     *plan = p;
     return DDSP_OK;
 }
@@ -171,20 +182,35 @@ int ddsp_plan_set_pitch(ddsp_plan* p, int64_t in_pitch, int64_t out_pitch) {
 
 int ddsp_plan_set_kernel(ddsp_plan* p, int kernel) {
     if (!p) return DDSP_ERR_INVALID_ARG;
-    if (kernel != DDSP_KERNEL_AUTO && kernel != DDSP_KERNEL_DIRECT && kernel != DDSP_KERNEL_TILED)
+    if (kernel != DDSP_KERNEL_AUTO && kernel != DDSP_KERNEL_DIRECT && kernel != DDSP_KERNEL_TILED &&
+        kernel != DDSP_KERNEL_LANES)
         return DDSP_ERR_INVALID_ARG;
     if (kernel == DDSP_KERNEL_TILED && !p->tiled.ok) return DDSP_ERR_UNSUPPORTED;
+    if (kernel == DDSP_KERNEL_LANES && !p->lanes.ok) return DDSP_ERR_UNSUPPORTED;
     p->kernel_req = kernel;
     resolve_kernel(p);
-    return DDSP_OK;
+    return p->kernel == DDSP_KERNEL_LANES ? ddsp_lanes_prepare(p) : DDSP_OK;
 }
 
 int64_t ddsp_plan_nsamp_out(const ddsp_plan* p) { return p ? p->nsamp_out : -1; }
 int64_t ddsp_plan_max_delay(const ddsp_plan* p) { return p ? p->dmax : -1; }
 int ddsp_plan_nchan_unmasked(const ddsp_plan* p) { return p ? (int)p->chan_list.size() : -1; }
 int ddsp_plan_kernel(const ddsp_plan* p) { return p ? p->kernel : -1; }
-int ddsp_plan_launches_per_execute(const ddsp_plan* p) { return p ? 1 : -1; }
-int ddsp_last_cuda_error(const ddsp_plan* p) { return p ? p->last_cuda : 0; }
+int ddsp_plan_launches_per_execute(const ddsp_plan* p) {
+    if (!p) return -1;
+    return p->kernel == DDSP_KERNEL_LANES ? (p->chan_list.empty() ? 1 : 2) : 1;   // interleave + accumulate
+}
+int64_t ddsp_plan_workspace_bytes(const ddsp_plan* p) {
+    if (!p) return -1;
+    return p->kernel == DDSP_KERNEL_LANES ? (int64_t)p->lanes.ws_bytes : 0;
+}
+int ddsp_plan_device_status(ddsp_plan* p, int* status) {
+    if (!p || !status) return DDSP_ERR_INVALID_ARG;
+    *status = 0;
+    if (p->device < 0 || !p->lanes.d_status) return DDSP_OK;
+    return note_cuda(p, cudaMemcpy(status, p->lanes.d_status, sizeof(int), cudaMemcpyDeviceToHost));
+}
+int ddsp_last_cuda_error(const ddsp_plan* p) { return p ? p->last_cuda.load() : 0; }
 
 int ddsp_plan_get_delays(const ddsp_plan* p, int32_t* host_out) {
     if (!p || !host_out) return DDSP_ERR_INVALID_ARG;
@@ -193,11 +219,19 @@ int ddsp_plan_get_delays(const ddsp_plan* p, int32_t* host_out) {
 }
 
 int ddsp_execute(const ddsp_plan* p, const void* d_in, void* d_out, void* cuda_stream) {
+    return ddsp_execute_ws(p, d_in, d_out, nullptr, 0, cuda_stream);
+}
+
+int ddsp_execute_ws(const ddsp_plan* p, const void* d_in, void* d_out, void* d_ws, int64_t ws_bytes,
+                    void* cuda_stream) {
     if (!p || !d_in || !d_out) return DDSP_ERR_INVALID_ARG;
     if (p->device < 0) return DDSP_ERR_CUDA;  // host-only plan: no device, no fallback
     cudaStream_t s = (cudaStream_t)cuda_stream;
     cudaError_t e;
-    if (p->kernel == DDSP_KERNEL_TILED && !ddsp_tiled_can_run(p, d_in, d_out)) {
+    if (p->kernel == DDSP_KERNEL_LANES) {
+        if (d_ws && (ws_bytes < (int64_t)p->lanes.ws_bytes || ((uintptr_t)d_ws & 15u))) return DDSP_ERR_INVALID_ARG;
+        e = ddsp_launch_lanes(p, d_in, d_out, d_ws, s);
+    } else if (p->kernel == DDSP_KERNEL_TILED && !ddsp_tiled_can_run(p, d_in, d_out)) {
         // unaligned buffers: correct through the direct kernel unless the tiled one was forced
         if (p->kernel_req == DDSP_KERNEL_TILED) return DDSP_ERR_UNSUPPORTED;
         e = ddsp_launch_direct(p, d_in, d_out, s);
@@ -232,6 +266,7 @@ int ddsp_execute_host(ddsp_plan* p, const void* h_in, void* h_out, void* cuda_st
 int ddsp_plan_destroy(ddsp_plan* p) {
     if (!p) return DDSP_OK;
     ddsp_tiled_free(p);
+    ddsp_lanes_free(p);
     if (p->d_delays) cudaFree(p->d_delays);
     if (p->d_chan_list) cudaFree(p->d_chan_list);
     if (p->d_stage_in) cudaFree(p->d_stage_in);

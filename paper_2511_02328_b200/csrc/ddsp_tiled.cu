@@ -26,6 +26,9 @@
 #include <vector>
 
 #include "ddsp_internal.h"
+#include "ddsp_dev.cuh"
+
+using namespace ddsp_dev;
 
 namespace {
 
@@ -49,14 +52,6 @@ struct TiledArgs {
     int nlist, nch_pad, nblk, chunk_shift, nchunk, row_stride, out_vec, in_vec;
 };
 
-__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
-    uint32_t v;
-    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ void lds128(uint32_t addr, uint32_t* v) {
-    asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]) : "r"(addr));
-}
 // ------------------------------------------------------------------------------------------------
 // uint8, ds = 1
 // ------------------------------------------------------------------------------------------------
@@ -81,7 +76,7 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
     const int chunk_c = 1 << a.chunk_shift;
     const int stage_rows_bytes = chunk_c * 4 * a.row_stride;
     const int stage_bytes = stage_rows_bytes + chunk_c * BDM * 4;
-    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t smem_base = smem_addr(smem);
 
     const int64_t* __restrict__ meta_b = a.meta + (size_t)blk * a.nch_pad;
     const uint32_t* __restrict__ off_b = a.off + (size_t)blk * a.nch_pad * BDM;

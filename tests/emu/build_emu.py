@@ -1,9 +1,10 @@
-"""Build the CPU emulation of the ring kernels (test infrastructure; see tests/test_ring_emulated_cpu.py).
+"""Build the CPU emulation of the library's kernels (test infrastructure; see tests/test_emulated_cpu.py).
 
-The product sources ddsp_plan.cpp, ddsp_ring.cu and ddsp_ringx.cu are compiled UNCHANGED except for three
-textual substitutions that g++ cannot do without: the `<<<...>>>` launch becomes a call of emu_launch, the
+The product sources (ddsp_plan.cpp and every .cu) are compiled UNCHANGED except for three textual
+substitutions that g++ cannot do without: the `<<<...>>>` launch becomes a call of emu_launch, the
 `extern __shared__` array becomes a pointer to the emulated CTA's buffer, and the include of the PTX helper
-header is redirected to its host stand-in (emu_common.h).  <cuda_runtime.h> resolves to the fake one here.
+header (ddsp_dev.cuh) is redirected to its host stand-in (emu_common.h).  <cuda_runtime.h> resolves to the
+fake one here.
 
     python tests/emu/build_emu.py [--tsan]   ->  tests/emu/build/libddsp_emu.so  (or emu_tsan, an executable)
 """
@@ -16,25 +17,21 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(os.path.dirname(HERE))
 CSRC = os.path.join(ROOT, "paper_2511_02328_b200", "csrc")
 BUILD = os.path.join(HERE, "build")
-PRODUCT = ["ddsp_plan.cpp", "ddsp_tiled.cu", "ddsp_direct.cu"]
+PRODUCT = ["ddsp_plan.cpp", "ddsp_lanes.cu", "ddsp_tiled.cu", "ddsp_direct.cu"]
 LIB = os.path.join(BUILD, "libddsp_emu.so")
 TSAN_EXE = os.path.join(BUILD, "emu_tsan")
 
 
 def transform(text):
+    # kernels without shared memory or barriers (the interleave pass): CUDA threads run one after another
+    text, n0 = re.subn(r"(kPreKernels\[[^\]]*\])<<<\s*([^;]*?)\s*>>>\(", r"emu_launch_v(\1, \2, ", text)
     text, n1 = re.subn(r"(\w[\w\[\]\.]*)<<<\s*([^;]*?)\s*>>>\((\w+)\);", r"emu_launch(\1, \2, \3);", text)
+    n1 += n0
     # launches with an argument list (template kernels of ddsp_direct.cu)
     text, n1b = re.subn(r"(\w+<[^;<>]*>)<<<\s*([^;]*?)\s*>>>\(", r"emu_launch_v(\1, \2, ", text)
     n1 += n1b
     text, n2 = re.subn(r"extern __shared__ __align__\(\d+\) uint8_t smem\[\];", "uint8_t* const smem = emu::smem();", text)
-    text = text.replace('#include "ddsp_ring_common.cuh"', '#include "emu_common.h"')
-    # ddsp_tiled.cu (the kernel already verified on hardware; here it calibrates the emulation) keeps its PTX
-    # helpers in the file: cut them out and use the same host stand-ins
-    m = re.search(r"__device__ __forceinline__ uint32_t lds32\(uint32_t addr\) \{.*?mad\.wide\.u32.*?\n\}\n", text, flags=re.S)
-    if m:
-        text = text[:m.start()] + "using namespace ddsp_dev;\n" + text[m.end():]
-        text = text.replace('#include "ddsp_internal.h"', '#include "ddsp_internal.h"\n#include "emu_common.h"', 1)
-        text = text.replace("(uint32_t)__cvta_generic_to_shared(smem)", "smem_addr(smem)")
+    text = text.replace('#include "ddsp_dev.cuh"', '#include "emu_common.h"')
     return text, n1, n2
 
 

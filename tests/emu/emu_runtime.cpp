@@ -1,7 +1,9 @@
 // Runtime of the CPU emulation harness: one std::thread per CUDA thread of a CTA, CTAs one after another,
-// a copy-engine thread for cp.async.bulk, mbarriers with the PTX counting rules.  Alignment and size rules of
-// the real instructions are asserted (16-byte bulk copies, 8-byte mbarriers, aligned vector accesses are the
-// callers' business).  Test infrastructure only.
+// a copy-engine thread for cp.async.bulk, mbarriers with the PTX counting rules.  The alignment and size rules
+// of the real instructions are checked (16-byte bulk copies, 8-byte mbarriers, aligned vector accesses), and so
+// is the RANGE of every access: shared-memory accesses against the CTA's dynamic shared memory, global accesses
+// and bulk-copy sources against the registered device-memory extents (cudaMalloc stand-in + ddsp_emu_register).
+// Test infrastructure only.
 #include <pthread.h>
 #include <unistd.h>
 
@@ -49,12 +51,18 @@ struct Cta {
     std::atomic<long> faults{0};
 };
 Cta* cta = nullptr;
-long total_faults = 0;
+std::atomic<long> total_faults{0};
+std::atomic<long> printed{0};
 
 void fault(const char* what, long a = 0, long b = 0) {
-    std::fprintf(stderr, "EMU FAULT: %s (%ld, %ld)\n", what, a, b);
-    ++cta->faults;
+    if (printed.fetch_add(1) < 20) std::fprintf(stderr, "EMU FAULT: %s (%ld, %ld)\n", what, a, b);
+    if (cta) ++cta->faults; else ++total_faults;
 }
+
+// registered device-memory extents: changed only between launches (cudaMalloc / cudaFree / register)
+struct Extent { uintptr_t lo, hi; };
+std::mutex ext_mutex;
+std::vector<Extent> extents;
 
 // pending -= arrivals, tx += dtx; the phase completes when both reach zero
 bool update(MBar& m, int arrivals, int64_t dtx) {
@@ -85,6 +93,7 @@ void engine_main(int delay_us) {
             cta->queue.pop_front();
         }
         if (delay_us > 0) usleep(delay_us);
+        check_global(c.src, c.bytes, false);
         std::memcpy(cta->smem.data() + c.dst, c.src, c.bytes);
         update(cta->mbar[c.bar / 8], 0, -(int64_t)c.bytes);
     }
@@ -93,6 +102,39 @@ void engine_main(int delay_us) {
 }  // namespace
 
 uint8_t* smem() { return cta->smem.data(); }
+
+uint8_t* smem_at(uint32_t addr, uint32_t n, uint32_t align) {
+    if ((size_t)addr + n > cta->smem_bytes) { fault("shared-memory access out of range", addr, n); return cta->smem.data() + cta->smem_bytes; }
+    if (addr % align) fault("misaligned shared-memory access", addr, align);
+    return cta->smem.data() + addr;
+}
+
+void* dev_alloc(size_t n) {
+    void* p = nullptr;
+    if (posix_memalign(&p, 256, n ? n : 1)) return nullptr;
+    std::lock_guard<std::mutex> l(ext_mutex);
+    extents.push_back(Extent{(uintptr_t)p, (uintptr_t)p + n});
+    return p;
+}
+void dev_free(void* p) {
+    if (!p) return;
+    {
+        std::lock_guard<std::mutex> l(ext_mutex);
+        for (size_t i = 0; i < extents.size(); ++i)
+            if (extents[i].lo == (uintptr_t)p) { extents.erase(extents.begin() + i); break; }
+    }
+    std::free(p);
+}
+void check_global(const void* p, size_t n, bool write) {
+    const uintptr_t a = (uintptr_t)p;
+    for (const Extent& e : extents)          // a handful of entries; only read while a launch is running
+        if (a >= e.lo && a + n <= e.hi) return;
+    fault(write ? "global WRITE outside every registered device buffer" : "global READ outside every registered device buffer",
+          (long)a, (long)n);
+}
+void check_aligned(const void* p, size_t align) {
+    if ((uintptr_t)p % align) fault("misaligned global vector access", (long)(uintptr_t)p, (long)align);
+}
 void yield() { std::this_thread::yield(); }
 
 void mbar_init(uint32_t bar, int count) {
@@ -116,6 +158,7 @@ bool mbar_test(uint32_t bar, uint32_t parity) {
 void bulk_copy(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
     if (dst % 16 || (uintptr_t)src % 16 || bytes % 16 || bytes == 0) fault("cp.async.bulk alignment/size", dst, bytes);
     if ((size_t)dst + bytes > cta->smem_bytes) { fault("cp.async.bulk beyond shared memory", dst, bytes); return; }
+    check_global(src, bytes, false);
     std::lock_guard<std::mutex> l(cta->q_mutex);
     cta->queue.push_back(Copy{dst, src, bytes, bar});
 }
@@ -130,7 +173,23 @@ unsigned shfl_xor(unsigned v, int lane_mask) {
     return r;
 }
 
-long faults() { return total_faults; }
+long faults() { return total_faults.load(); }
+
+void launch_seq(unsigned grid, unsigned nthreads, const std::function<void()>& body) {
+    const unsigned nworkers = std::max(1u, std::min(8u, std::thread::hardware_concurrency()));
+    std::atomic<unsigned> next{0};
+    std::vector<std::thread> th;
+    for (unsigned w = 0; w < nworkers; ++w)
+        th.emplace_back([&]() {
+            for (unsigned b = next.fetch_add(1); b < grid; b = next.fetch_add(1))
+                for (unsigned t = 0; t < nthreads; ++t) {
+                    ctx.tid = t;
+                    ctx.bid = b;
+                    body();
+                }
+        });
+    for (auto& t : th) t.join();
+}
 
 void launch(unsigned grid, unsigned nthreads, size_t smem_bytes, const std::function<void()>& body) {
     const char* d = getenv("DDSP_EMU_TMA_DELAY_US");
@@ -174,3 +233,14 @@ void launch(unsigned grid, unsigned nthreads, size_t smem_bytes, const std::func
 }  // namespace emu
 
 extern "C" long ddsp_emu_faults(void) { return emu::faults(); }
+// caller-owned "device" buffers (the tests' input / output arrays): exact extents, so that a kernel that reads or
+// writes one byte outside them is reported
+extern "C" void ddsp_emu_register(const void* p, size_t n) {
+    std::lock_guard<std::mutex> l(emu::ext_mutex);
+    emu::extents.push_back(emu::Extent{(uintptr_t)p, (uintptr_t)p + n});
+}
+extern "C" void ddsp_emu_unregister(const void* p) {
+    std::lock_guard<std::mutex> l(emu::ext_mutex);
+    for (size_t i = 0; i < emu::extents.size(); ++i)
+        if (emu::extents[i].lo == (uintptr_t)p) { emu::extents.erase(emu::extents.begin() + i); break; }
+}
