@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- headline measurement of the dedispersion hot path (BASELINE.json metric).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config fast] [--kernel auto|direct|tiled]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config fast] [--kernel auto|direct|tiled|lanes]
     python bench.py --impl reference ...          # the CPU oracle on the host cores, same metric
 
 A "step" is one pass of the whole hot path (ddsp_execute: stage, fused bin-sum, shifted accumulate,
@@ -9,6 +9,10 @@ write-out) over one synthetic observation.  At N = 1 the workload is BASELINE.js
 ("FAST-like": 2048 channels, 150 s, 1001 DM trials).  With N > 1 (torchrun, one rank per GPU) every
 rank dedisperses its own observation of that shape -- independent units, no collective on the data
 path (weak scaling).  One JSON line is printed by rank 0.
+
+The kernel that runs is the LIBRARY's choice (`--kernel auto` = ddsp's AUTO); bench.py never picks, races or
+sweeps kernels.  A result that differs from the oracle on the compared sample, or an end-to-end result that
+differs from the device result, prints an error line and exits non-zero: a wrong kernel publishes no number.
 """
 import argparse
 import json
@@ -26,7 +30,9 @@ if ROOT not in sys.path:
 
 METRIC = "dedispersion_gadds_per_s"
 UNIT = "Gadd/s (DM x chan x sample)"
-SM_COUNT, SM_MAX_MHZ, ADDS_PER_CLK_SM = 148, 1965.0, 128   # DESIGN.md section 7: P_add
+SM_COUNT, SM_MAX_MHZ, ADDS_PER_CLK_SM = 148, 1965.0, 128   # DESIGN.md section 6.6: P_add
+KERNEL_IDS = {"auto": 0, "direct": 1, "tiled": 2, "lanes": 3}
+KERNEL_NAMES = {1: "direct", 2: "tiled", 3: "lanes"}
 
 
 def parse_args():
@@ -36,12 +42,10 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="fast", help="workload name (synth.CONFIG_NAMES); headline = fast")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "direct", "tiled"])
+    ap.add_argument("--kernel", default="auto", choices=sorted(KERNEL_IDS))
     ap.add_argument("--crop", type=int, default=0, help="debug: crop to this many output samples")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--traffic-bytes", type=float, default=None,
-                    help="dram bytes per launch of the dominant kernel from an ncu capture (profiles/)")
     return ap.parse_args()
 
 
@@ -112,38 +116,79 @@ def library_native_delays(wl):
 
 def get_workload(args):
     from paper_2511_02328_b200 import synth
-    wl = synth.config(args.config)
-    return wl
+    return synth.config(args.config)
 
 
 def adds_per_execute(plan):
     return float(plan.ndm) * float(plan.nchan_unmasked) * float(plan.nsamp_out)
 
 
-def oracle_sample(wl, x_dev_or_host, plan_geom, target_adds=1.6e10, ntrials=8):
-    """Bounded sample of the same workload for the CPU oracle: all channels, `ntrials` evenly spaced
-    trials, the first `ncol` output columns.  Returns (rows, ncol, host input window)."""
-    nout, dmax, nch_un = plan_geom
+def cpu_model():
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def oracle_sample(wl, x, nout, dmax, nch_un, ntrials, target_adds):
+    """Bounded sample of the same workload for the CPU oracle: all channels, `ntrials` evenly spaced trials,
+    the first `ncol` output columns.  Returns (rows, ncol, host input window)."""
     rows = np.unique(np.linspace(0, wl.ndm - 1, ntrials).round().astype(np.int64))
     ncol = int(min(nout, max(1024, target_adds / (len(rows) * max(1, nch_un)))))
     ncols_in = min(wl.nsamp, (ncol + dmax) * wl.downsample)
-    xh = x_dev_or_host[:, :ncols_in]
+    xh = x[:, :ncols_in]
     xh = xh.cpu().numpy() if hasattr(xh, "cpu") else np.ascontiguousarray(xh)
     return rows, ncol, np.ascontiguousarray(xh)
 
 
-def time_oracle(wl, rows, ncol, xh, dmax):
-    """Run the oracle (as it stands, single thread) on the sample; returns (seconds, output, adds)."""
+def run_oracle(wl, table, rows, ncol, xh, nthreads):
+    """The oracle as it stands (a single-threaded C++ triple loop) on the sample.  nthreads > 1: the SAME
+    function is called on disjoint DM-row ranges from one thread per host core (SURVEY.md 8(d) 'all-core
+    figure'); ctypes releases the GIL.  Returns (seconds, output, adds, threads used)."""
     from oracle import oracle
-    table, dmax_o = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, wl.downsample)
-    assert dmax_o == dmax
-    nsamp_win = xh.shape[1]
+    parts = [p for p in np.array_split(np.arange(len(rows)), nthreads) if len(p)]
+    outs = [None] * len(parts)
+
+    def work(k):
+        outs[k] = oracle.dedisperse_table(xh, table[rows[parts[k]]], nsamp=xh.shape[1], downsample=wl.downsample,
+                                          mask=wl.mask, t_lo=0, t_hi=ncol)
+    threads = [threading.Thread(target=work, args=(k,)) for k in range(len(parts))]
     t0 = time.perf_counter()
-    out = oracle.dedisperse_table(xh, table[rows], nsamp=nsamp_win, downsample=wl.downsample,
-                                  mask=wl.mask, t_lo=0, t_hi=ncol)
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
     dt = time.perf_counter() - t0
     nch_un = wl.nchan - (0 if wl.mask is None else int(wl.mask.sum()))
-    return dt, out, float(len(rows)) * nch_un * ncol
+    return dt, np.concatenate(outs, axis=0), float(len(rows)) * nch_un * ncol, len(parts)
+
+
+def profile_traffic(kernel, config):
+    """dram bytes per launch of the dominant kernel from the committed ncu summary (profiles/traffic.json, written
+    by paper_2511_02328_b200/ncu_summary.py from `ncu --page raw --csv`), or None if that kernel / config has no
+    capture yet."""
+    try:
+        table = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+    except (OSError, ValueError):
+        return None, None
+    e = table.get("%s/%s" % (kernel, config))
+    return (float(e["dram_bytes_per_launch"]), e.get("source")) if e else (None, None)
+
+
+def fail(what, **kw):
+    print(json.dumps(dict({"metric": METRIC, "value": None, "unit": UNIT, "error": what}, **kw)))
+    sys.stdout.flush()
+    sys.exit(3)
 
 
 # ----------------------------------------------------------------------------------------------
@@ -167,7 +212,7 @@ def run_ours(args):
     if args.crop:
         with binding.plan_for(wl) as geom:
             wl = wl.cropped(wl.downsample * (geom.max_delay + args.crop))
-    # every rank owns whole observations (units); rank r's observation uses seed + r
+    # every rank owns whole observations (units); rank r's observation uses seed + 1000 r
     unit = list(multi.shard_units(world, rank, world))[0]
     wl.seed = wl.seed + 1000 * unit
 
@@ -175,13 +220,15 @@ def run_ours(args):
     in_pitch = synth.round_up(wl.nsamp, 128)
     out_pitch = synth.round_up(plan.nsamp_out, 32)
     plan.set_pitch(in_pitch, out_pitch)
-    plan.set_kernel({"auto": 0, "direct": 1, "tiled": 2}[args.kernel])
+    plan.set_kernel(KERNEL_IDS[args.kernel])          # "auto": the library's AUTO, nothing else
+    kernel = KERNEL_NAMES[plan.kernel]
     x = synth.make_input(wl, dev, pitch=in_pitch, native_delays=library_native_delays(wl),
                          nsamp_out=plan.nsamp_out)
     out = torch.empty((plan.ndm, out_pitch), dtype=torch.int32 if wl.dtype == "u8" else torch.float32,
                       device=dev)
     stream = torch.cuda.current_stream(dev)
     adds = adds_per_execute(plan)
+
     for _ in range(max(args.warmup, 0)):
         plan.execute(x, out, stream)
     torch.cuda.synchronize(dev)
@@ -202,6 +249,10 @@ def run_ours(args):
     clocks = sampler.window(t_wall0, t_wall1) if sampler else None
     if sampler:
         sampler.stop()
+    status = plan.device_status()
+    if status != 0:
+        fail("device status %d after the timed region (1: a bounded barrier wait ran out, 2: table bounds check)"
+             % status, kernel=kernel)
 
     total_rate, t_max = multi.job_throughput(adds * args.steps, secs)      # adds/s over all ranks
     ms_per_step = t_max / args.steps * 1e3
@@ -209,12 +260,13 @@ def run_ours(args):
     # end to end through the public host-buffer call (H2D + kernels + D2H inside the timed region)
     e2e = None
     if not args.no_e2e:
-        e2e = measure_e2e(plan, wl, x, out, in_pitch, out_pitch, adds, min(args.steps, 3), multi)
+        e2e = measure_e2e(plan, wl, x, out, adds, min(args.steps, 3), multi)
+        if e2e.get("matches_device_result") is False:
+            fail("end-to-end result differs from the device result", kernel=kernel)
 
     result = None
     if rank == 0:
         p_add = SM_COUNT * ADDS_PER_CLK_SM * SM_MAX_MHZ * 1e6                 # adds/s
-        launch_s = secs / args.steps / plan.launches_per_execute
         achieved = adds / (secs / args.steps)
         peaks = {}
         try:
@@ -224,6 +276,7 @@ def run_ours(args):
         hbm = float(peaks.get("hbm_gbs", 6650.0)) * 1e9
         ideal_bytes = float(wl.nchan) * wl.nsamp * wl.elem_size + float(plan.ndm) * plan.nsamp_out * 4
         t_roof = max(ideal_bytes / hbm, adds / p_add)
+        traffic, traffic_src = profile_traffic(kernel, wl.name)
         result = {
             "metric": METRIC, "value": total_rate / 1e9, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
@@ -232,34 +285,53 @@ def run_ours(args):
             "config": {"workload": "%s%s" % (wl.name, "" if not args.crop else "(cropped)"),
                        "nchan": wl.nchan, "nchan_unmasked": plan.nchan_unmasked, "ndm": plan.ndm,
                        "nsamp": wl.nsamp, "nsamp_out": plan.nsamp_out, "tsamp_s": wl.tsamp,
-                       "downsample": wl.downsample, "in_dtype": wl.dtype,
-                       "kernel": {1: "direct", 2: "tiled"}[plan.kernel],
+                       "downsample": wl.downsample, "in_dtype": wl.dtype, "kernel": kernel,
+                       "launches_per_execute": plan.launches_per_execute,
+                       "workspace_bytes": plan.workspace_bytes,
                        "units": "one observation per GPU", "parallelism": "dp%d" % world,
                        "l2": "inputs (%.2f GB) larger than L2; no flush" % (x.numel() * x.element_size() / 1e9)},
             "x_realtime": plan.nsamp_out * wl.tsamp * wl.downsample / (t_max / args.steps),
             "gpu_launches": args.steps * plan.launches_per_execute,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved / 1e9, "peak": p_add / 1e9, "unit": "Gadd/s",
-                         "frac": achieved / p_add, "traffic": args.traffic_bytes,
-                         "peak_source": "148 SM x 128 int32 adds/clk/SM (measured, profiles/ubench_r01_raw.txt) x 1965 MHz",
-                         "kernel_ms": launch_s * 1e3,
+                         "frac": achieved / p_add, "traffic": traffic, "traffic_source": traffic_src,
+                         "peak_source": "148 SM x 128 32-bit integer adds/clk/SM x 1965 MHz (DESIGN.md 6.6; issue "
+                                        "rates: paper_2511_02328_b200/ubench.py, table in profiles/)",
+                         "execute_ms": secs / args.steps * 1e3,
                          "t_roof_ms": t_roof * 1e3, "frac_of_path_roofline": t_roof / (secs / args.steps),
                          "hbm_ideal_bytes": ideal_bytes, "hbm_peak_gbs": hbm / 1e9,
                          "hbm_peak_source": "measured" if peaks else "fallback"},
             "e2e": e2e,
         }
-        if not args.no_cpu_baseline and world >= 1:
-            rows, ncol, xh = oracle_sample(wl, x, (plan.nsamp_out, plan.max_delay, plan.nchan_unmasked))
-            dt, oout, oadds = time_oracle(wl, rows, ncol, xh, plan.max_delay)
+        if not args.no_cpu_baseline:
+            from oracle import oracle
+            table, dmax_o = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, wl.downsample)
+            assert dmax_o == plan.max_delay
+            ncores = host_cores()
+            # (i) one thread, 8 evenly spaced trials: also the parity sample of the timed launch configuration
+            rows, ncol, xh = oracle_sample(wl, x, plan.nsamp_out, plan.max_delay, plan.nchan_unmasked, 8, 1.6e10)
+            dt1, oout, oadds1, _ = run_oracle(wl, table, rows, ncol, xh, 1)
             got = out[torch.as_tensor(rows, device=dev), :ncol].cpu().numpy()
             if wl.dtype == "u8":
                 ok = bool(np.array_equal(got.view(np.uint32), oout))
             else:
                 ok = bool((np.abs(got.astype(np.float64) - oout) <= 1e-5 * np.abs(oout)).all())
-            result["cpu_baseline"] = {"value": oadds / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                      "sample": "%d trials x %d channels x first %d output samples of the same "
-                                                "input (%.1f s of CPU)" % (len(rows), plan.nchan_unmasked, ncol, dt),
-                                      "parity_on_sample": "ok" if ok else "MISMATCH"}
+            if not ok:
+                fail("the CUDA result differs from the oracle on the sample (%d trials x first %d columns)"
+                     % (len(rows), ncol), kernel=kernel)
+            # (ii) all cores: the same function on disjoint DM-row ranges, one thread per core
+            rows_n, ncol_n, xh_n = oracle_sample(wl, x, plan.nsamp_out, plan.max_delay, plan.nchan_unmasked,
+                                                 max(8, 4 * ncores), 1.2e10 * max(1, ncores) ** 0.5)
+            dtn, _, oaddsn, used = run_oracle(wl, table, rows_n, ncol_n, xh_n, ncores)
+            result["cpu_baseline"] = {
+                "value": oaddsn / dtn / 1e9, "unit": UNIT, "cores": used, "kind": "oracle", "cpu": cpu_model(),
+                "sample": "%d trials x %d channels x first %d output samples of the same input, the unchanged "
+                          "single-threaded oracle on disjoint DM rows in %d threads (%.1f s)"
+                          % (len(rows_n), plan.nchan_unmasked, ncol_n, used, dtn),
+                "single_thread": {"value": oadds1 / dt1 / 1e9, "cores": 1,
+                                  "sample": "%d trials x %d channels x first %d output samples (%.1f s)"
+                                            % (len(rows), plan.nchan_unmasked, ncol, dt1)},
+                "parity_on_sample": "ok"}
         print(json.dumps(result))
         sys.stdout.flush()
     plan.destroy()
@@ -267,7 +339,7 @@ def run_ours(args):
     return result
 
 
-def measure_e2e(plan, wl, x, out, in_pitch, out_pitch, adds, steps, multi):
+def measure_e2e(plan, wl, x, out, adds, steps, multi):
     """Same metric through ddsp_execute_host: pinned host input -> device, kernels, result -> pinned host."""
     import psutil
     import torch
@@ -277,17 +349,15 @@ def measure_e2e(plan, wl, x, out, in_pitch, out_pitch, adds, steps, multi):
     if psutil.virtual_memory().available < 1.5 * (in_bytes + out_bytes):
         return {"value": None, "unit": UNIT, "h2d_bytes_per_step": in_bytes, "d2h_bytes_per_step": valid_out_bytes,
                 "note": "skipped: not enough host memory to pin the buffers"}
-    # free the device-resident copies so that the plan's own staging buffers fit comfortably
     xh = torch.empty(x.shape, dtype=x.dtype, pin_memory=True)
     xh.copy_(x)
     oh = torch.empty(out.shape, dtype=out.dtype, pin_memory=True)
-    call, how = plan.execute_host, "ddsp_execute_host (copy in, kernel, copy out in sequence)"
-    call(xh, oh)                                   # warm-up: allocates the staging buffers
+    plan.execute_host(xh, oh)                      # warm-up: allocates the staging buffers
     torch.cuda.synchronize()
     multi.barrier()
     t0 = time.perf_counter()
     for _ in range(steps):
-        call(xh, oh)                               # synchronises before returning
+        plan.execute_host(xh, oh)                  # synchronises before returning
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     rate, t_max = multi.job_throughput(adds * steps, dt)
@@ -295,7 +365,8 @@ def measure_e2e(plan, wl, x, out, in_pitch, out_pitch, adds, steps, multi):
     return {"value": rate / 1e9, "unit": UNIT, "h2d_bytes_per_step": in_bytes,
             "d2h_bytes_per_step": valid_out_bytes, "steps": steps, "ms_per_step": t_max / steps * 1e3,
             "x_realtime": plan.nsamp_out * wl.tsamp * wl.downsample / (t_max / steps),
-            "matches_device_result": same, "call": how}
+            "matches_device_result": same,
+            "call": "ddsp_execute_host (copy in, kernels, copy out in sequence)"}
 
 
 # ----------------------------------------------------------------------------------------------
@@ -305,7 +376,6 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return None
-    import torch
     from oracle import oracle
     from paper_2511_02328_b200 import synth
     oracle.build()
@@ -313,23 +383,21 @@ def run_reference(args):
     table, dmax = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, wl.downsample)
     nout = oracle.nsamp_ds(wl.nsamp, wl.downsample) - dmax
     nch_un = wl.nchan - (0 if wl.mask is None else int(wl.mask.sum()))
-    # bounded sample per step: 8 evenly spaced trials, all channels, a window of the observation
-    rows = np.unique(np.linspace(0, wl.ndm - 1, 8).round().astype(np.int64))
-    ncol = int(min(nout, max(1024, 4e9 / (len(rows) * max(1, nch_un)))))
+    ncores = host_cores()
+    # bounded sample per step: evenly spaced trials (4 per core), all channels, a window of the observation
+    rows = np.unique(np.linspace(0, wl.ndm - 1, max(8, 4 * ncores)).round().astype(np.int64))
+    ncol = int(min(nout, max(1024, 4e9 * max(1, ncores) ** 0.5 / (len(rows) * max(1, nch_un)))))
     win = wl.cropped(min(wl.nsamp, (ncol + dmax) * wl.downsample))
     xh = synth.make_input(win, "cpu", native_delays=lambda dm: oracle.delay_table(
         wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, [dm], 1)[0][0], nsamp_out=nout).numpy()
-    times = []
+    times, used, adds = [], 1, 0.0
     for it in range(args.warmup + args.steps):
-        t0 = time.perf_counter()
-        oracle.dedisperse_table(xh, table[rows], nsamp=win.nsamp, downsample=wl.downsample, mask=wl.mask,
-                                t_lo=0, t_hi=ncol)
+        dt, _, adds, used = run_oracle(wl, table, rows, ncol, xh, ncores)
         if it >= args.warmup:
-            times.append(time.perf_counter() - t0)
-    adds = float(len(rows)) * nch_un * ncol
+            times.append(dt)
     secs = sum(times)
     value = adds * args.steps / secs / 1e9
-    sample = "%d trials x %d channels x %d output samples per step" % (len(rows), nch_un, ncol)
+    sample = "%d trials x %d channels x %d output samples per step, %d threads" % (len(rows), nch_un, ncol, used)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs / args.steps * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -337,7 +405,8 @@ def run_reference(args):
             "config": {"workload": wl.name, "nchan": wl.nchan, "ndm": wl.ndm, "nsamp": wl.nsamp,
                        "sample": sample},
             "gpu_launches": 0,
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "cpu": cpu_model(),
+                             "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
     return line

@@ -538,3 +538,31 @@ cudaError_t ddsp_launch_lanes(const ddsp_plan* p, const void* d_in, void* d_out,
     kLanesKernels[g.kind]<<<grid, kThreads, g.smem_bytes, s>>>(a);
     return cudaGetLastError();
 }
+
+#ifdef DDSP_TESTING
+// Introspection for the CPU tests (include/ddsp_testing.h); not part of the product library.
+#include "../../include/ddsp_testing.h"
+#include <cstring>
+
+extern "C" int ddsp_testing_lanes_geometry(const ddsp_plan* p, int64_t* geom) {
+    if (!p || !geom) return DDSP_ERR_INVALID_ARG;
+    const ddsp_lanes& g = p->lanes;
+    if (!g.ok) return DDSP_ERR_UNSUPPORTED;
+    int64_t NT, Q, M;
+    ddsp_lanes_range(p, p->nsamp_out, &NT, &Q, &M);
+    const int64_t v[16] = {g.kind, kLanesPerWord[g.kind], kWordBytes[g.kind], kBDM, kTW, kC, g.nblk, g.nchunk, g.RS,
+                           g.NS, g.stage_bytes, g.smem_bytes, g.flush_rows, NT, Q, M};
+    std::memcpy(geom, v, sizeof(v));
+    return DDSP_OK;
+}
+
+extern "C" int ddsp_testing_lanes_tables(const ddsp_plan* p, int32_t* win, uint32_t* off, int32_t* rows) {
+    if (!p || !win || !off || !rows) return DDSP_ERR_INVALID_ARG;
+    const ddsp_lanes& g = p->lanes;
+    if (!g.ok) return DDSP_ERR_UNSUPPORTED;
+    for (size_t i = 0; i < g.h_win.size(); ++i) { win[2 * i] = g.h_win[i].x; win[2 * i + 1] = g.h_win[i].y; }
+    std::memcpy(off, g.h_off.data(), g.h_off.size() * sizeof(uint32_t));
+    std::memcpy(rows, g.h_rows.data(), g.h_rows.size() * sizeof(int32_t));
+    return DDSP_OK;
+}
+#endif  // DDSP_TESTING

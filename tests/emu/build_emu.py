@@ -70,7 +70,7 @@ def build(tsan=False, mutate=None):
             f.write(text)
         srcs.append(out)
     srcs += [os.path.join(HERE, "emu_runtime.cpp")]
-    flags = ["-std=c++17", "-O1", "-g", "-fPIC", "-pthread", "-ffp-contract=off", "-fno-fast-math", "-w",
+    flags = ["-std=c++17", "-O1", "-g", "-fPIC", "-pthread", "-ffp-contract=off", "-fno-fast-math", "-w", "-DDDSP_TESTING",
              "-I", HERE, "-I", CSRC, "-I", os.path.join(ROOT, "include")]
     if tsan:
         cmd = ["g++"] + flags + ["-fsanitize=thread"] + srcs + [os.path.join(HERE, "emu_tsan_main.cpp"), "-o", target]

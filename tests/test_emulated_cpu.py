@@ -261,3 +261,32 @@ def test_negative_control_input_too_small(emu, oracle):
         out.release()
     finally:
         emu.ddsp_plan_destroy(h)
+
+
+# ---- race check of the shared-memory protocol under ThreadSanitizer (tests/emu/emu_tsan_main.cpp) -------------
+def _run_tsan(exe, case, halt=0):
+    env = dict(os.environ, TSAN_OPTIONS="halt_on_error=%d report_signal_unsafe=0" % halt)
+    r = subprocess.run([exe, case], capture_output=True, text=True, timeout=900, env=env)
+    if "FATAL: ThreadSanitizer" in r.stderr:        # e.g. an address-space layout the sanitizer runtime rejects
+        pytest.skip("ThreadSanitizer cannot run here: " + r.stderr.strip().splitlines()[0])
+    return r
+
+
+@pytest.mark.parametrize("case", ["u8", "bins2", "bins4", "f32"])
+def test_lanes_protocol_is_race_free(case):
+    """More chunks than ring stages and several work items per CTA, so every stage is refilled by the copy engine
+    while other warps are still at work on its neighbours: no shared-memory access may be unordered with
+    respect to the copy engine."""
+    r = _run_tsan(build_emu.build(tsan=True), case)
+    assert "ThreadSanitizer" not in r.stderr, r.stderr[-3000:]
+    assert r.returncode == 0, (r.stdout, r.stderr[-2000:])
+    assert "faults=0" in r.stdout and "status=0" in r.stdout
+
+
+def test_lanes_race_check_can_fail():
+    """Negative control: a producer that refills a stage WITHOUT waiting for the consumers' `empty` barrier must be
+    reported as a data race -- otherwise the clean runs above would prove nothing."""
+    exe = build_emu.build(tsan=True, mutate=("early", "if (p_issued >= a.NS) ok = mbar_wait(", "if (false) ok = mbar_wait(",
+                                              "ddsp_lanes.cu"))
+    r = _run_tsan(exe, "u8", halt=1)          # the first report ends the run
+    assert "ThreadSanitizer: data race" in r.stderr
