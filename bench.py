@@ -43,6 +43,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="fast", help="workload name (synth.CONFIG_NAMES); headline = fast")
     ap.add_argument("--kernel", default="auto", choices=sorted(KERNEL_IDS))
+    ap.add_argument("--split", default="obs", choices=["obs", "dm"],
+                    help="N > 1: 'obs' = one whole observation per GPU (weak scaling, no exchange); 'dm' = ONE "
+                         "observation, DM rows sharded over the GPUs after one NCCL broadcast of the input (strong)")
     ap.add_argument("--crop", type=int, default=0, help="debug: crop to this many output samples")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -140,10 +143,11 @@ def host_cores():
         return os.cpu_count() or 1
 
 
-def oracle_sample(wl, x, nout, dmax, nch_un, ntrials, target_adds):
-    """Bounded sample of the same workload for the CPU oracle: all channels, `ntrials` evenly spaced trials,
-    the first `ncol` output columns.  Returns (rows, ncol, host input window)."""
-    rows = np.unique(np.linspace(0, wl.ndm - 1, ntrials).round().astype(np.int64))
+def oracle_sample(wl, x, nout, dmax, nch_un, ntrials, target_adds, row_range=None):
+    """Bounded sample of the same workload for the CPU oracle: all channels, `ntrials` evenly spaced trials (of
+    this rank's row range), the first `ncol` output columns.  Returns (rows, ncol, host input window)."""
+    lo, cnt = (0, wl.ndm) if row_range is None else row_range
+    rows = np.unique(np.linspace(lo, lo + cnt - 1, ntrials).round().astype(np.int64))
     ncol = int(min(nout, max(1024, target_adds / (len(rows) * max(1, nch_un)))))
     ncols_in = min(wl.nsamp, (ncol + dmax) * wl.downsample)
     xh = x[:, :ncols_in]
@@ -212,18 +216,40 @@ def run_ours(args):
     if args.crop:
         with binding.plan_for(wl) as geom:
             wl = wl.cropped(wl.downsample * (geom.max_delay + args.crop))
-    # every rank owns whole observations (units); rank r's observation uses seed + 1000 r
-    unit = list(multi.shard_units(world, rank, world))[0]
-    wl.seed = wl.seed + 1000 * unit
+    split_dm = args.split == "dm" and world > 1
+    rows = None
+    if split_dm:
+        # ONE observation; rank r computes the contiguous DM-row range shard_rows(ndm, r, world)
+        rows = multi.shard_rows(wl.ndm, rank, world)
+        if rows[1] < 1:
+            raise SystemExit("bench.py: more ranks than DM rows")
+    else:
+        # every rank owns whole observations (units); rank r's observation uses seed + 1000 r
+        unit = list(multi.shard_units(world, rank, world))[0]
+        wl.seed = wl.seed + 1000 * unit
 
-    plan = binding.plan_for(wl)
+    rows_of_rank, row0 = rows, (rows[0] if rows else 0)
+    plan = binding.plan_for(wl, rows=rows)
     in_pitch = synth.round_up(wl.nsamp, 128)
     out_pitch = synth.round_up(plan.nsamp_out, 32)
     plan.set_pitch(in_pitch, out_pitch)
     plan.set_kernel(KERNEL_IDS[args.kernel])          # "auto": the library's AUTO, nothing else
     kernel = KERNEL_NAMES[plan.kernel]
-    x = synth.make_input(wl, dev, pitch=in_pitch, native_delays=library_native_delays(wl),
-                         nsamp_out=plan.nsamp_out)
+    if split_dm and rank != 0:
+        x = torch.empty((wl.nchan, in_pitch), dtype=wl.torch_dtype, device=dev)
+    else:
+        x = synth.make_input(wl, dev, pitch=in_pitch, native_delays=library_native_delays(wl),
+                             nsamp_out=plan.nsamp_out)
+    bcast_ms = None
+    if split_dm:                                      # the path's only exchange step: one broadcast of the input
+        torch.cuda.synchronize(dev)
+        multi.barrier()
+        b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b0.record()
+        multi.broadcast_input(x, src=0)
+        b1.record()
+        torch.cuda.synchronize(dev)
+        bcast_ms = multi.max_over_ranks(b0.elapsed_time(b1))
     out = torch.empty((plan.ndm, out_pitch), dtype=torch.int32 if wl.dtype == "u8" else torch.float32,
                       device=dev)
     stream = torch.cuda.current_stream(dev)
@@ -280,7 +306,7 @@ def run_ours(args):
         result = {
             "metric": METRIC, "value": total_rate / 1e9, "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "higher_is_better": True, "scaling": "strong" if split_dm else "weak", "vs_baseline": None,
             "dtype": "u32" if wl.dtype == "u8" else "f32", "data": "synthetic",
             "config": {"workload": "%s%s" % (wl.name, "" if not args.crop else "(cropped)"),
                        "nchan": wl.nchan, "nchan_unmasked": plan.nchan_unmasked, "ndm": plan.ndm,
@@ -288,7 +314,9 @@ def run_ours(args):
                        "downsample": wl.downsample, "in_dtype": wl.dtype, "kernel": kernel,
                        "launches_per_execute": plan.launches_per_execute,
                        "workspace_bytes": plan.workspace_bytes,
-                       "units": "one observation per GPU", "parallelism": "dp%d" % world,
+                       "units": "DM rows of one observation per GPU" if split_dm else "one observation per GPU",
+                       "parallelism": ("dm-rows%d" if split_dm else "dp%d") % world,
+                       "input_broadcast_ms": bcast_ms,
                        "l2": "inputs (%.2f GB) larger than L2; no flush" % (x.numel() * x.element_size() / 1e9)},
             "x_realtime": plan.nsamp_out * wl.tsamp * wl.downsample / (t_max / args.steps),
             "gpu_launches": args.steps * plan.launches_per_execute,
@@ -306,12 +334,12 @@ def run_ours(args):
         if not args.no_cpu_baseline:
             from oracle import oracle
             table, dmax_o = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, wl.downsample)
-            assert dmax_o == plan.max_delay
+            assert dmax_o == plan.max_delay        # also in a DM-row split: d_max is the whole list's
             ncores = host_cores()
             # (i) one thread, 8 evenly spaced trials: also the parity sample of the timed launch configuration
-            rows, ncol, xh = oracle_sample(wl, x, plan.nsamp_out, plan.max_delay, plan.nchan_unmasked, 8, 1.6e10)
+            rows, ncol, xh = oracle_sample(wl, x, plan.nsamp_out, plan.max_delay, plan.nchan_unmasked, 8, 1.6e10, rows_of_rank)
             dt1, oout, oadds1, _ = run_oracle(wl, table, rows, ncol, xh, 1)
-            got = out[torch.as_tensor(rows, device=dev), :ncol].cpu().numpy()
+            got = out[torch.as_tensor(rows - row0, device=dev), :ncol].cpu().numpy()
             if wl.dtype == "u8":
                 ok = bool(np.array_equal(got.view(np.uint32), oout))
             else:

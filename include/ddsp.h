@@ -75,6 +75,14 @@ DDSP_API int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top_mhz, dou
                      int64_t nsamp, const double* dm_list, int ndm, int downsample,
                      const uint8_t* chan_mask, int in_dtype);
 
+/* The same plan for a contiguous RANGE of the DM list: rows [row_begin, row_begin + row_count) of dm_list (ndm_all
+ * entries).  d_max, and with it nsamp_out, is taken over the WHOLE list, so the outputs of plans that split one
+ * list are row ranges of the output of the plan for the whole list (one observation, DM rows
+ * sharded over GPUs, no reduction).  The output has row_count rows; ddsp_plan_get_delays returns them only. */
+DDSP_API int ddsp_plan_create_rows(ddsp_plan** plan, int nchan, double f_top_mhz, double chan_bw_mhz, double tsamp_s,
+                          int64_t nsamp, const double* dm_list, int ndm_all, int row_begin, int row_count,
+                          int downsample, const uint8_t* chan_mask, int in_dtype);
+
 /* Row pitches in ELEMENTS (not bytes).  Defaults: in_pitch = nsamp, out_pitch = nsamp_out.
  * Any pitch >= the row length is correct; the fast path wants 16-byte aligned base pointers and
  * (pitch * element size) % 16 == 0. */

@@ -21,6 +21,7 @@ DDSP_KERNEL_AUTO, DDSP_KERNEL_DIRECT, DDSP_KERNEL_TILED, DDSP_KERNEL_LANES = 0, 
 _i, _i64, _f64, _vp, _cp = ctypes.c_int, ctypes.c_int64, ctypes.c_double, ctypes.c_void_p, ctypes.c_char_p
 SIGNATURES = {
     "ddsp_plan_create": (_i, [ctypes.POINTER(_vp), _i, _f64, _f64, _f64, _i64, _vp, _i, _i, _vp, _i]),
+    "ddsp_plan_create_rows": (_i, [ctypes.POINTER(_vp), _i, _f64, _f64, _f64, _i64, _vp, _i, _i, _i, _i, _vp, _i]),
     "ddsp_plan_set_pitch": (_i, [_vp, _i64, _i64]),
     "ddsp_plan_set_kernel": (_i, [_vp, _i]),
     "ddsp_plan_nsamp_out": (_i64, [_vp]),
@@ -75,20 +76,22 @@ class Plan:
     """ddsp_plan_create / ddsp_execute / ddsp_plan_destroy with the header's argument names."""
 
     def __init__(self, nchan, f_top_mhz, chan_bw_mhz, tsamp_s, nsamp, dm_list, downsample=1,
-                 chan_mask=None, in_dtype=DDSP_IN_U8):
+                 chan_mask=None, in_dtype=DDSP_IN_U8, rows=None):
+        """rows = (row_begin, row_count): ddsp_plan_create_rows, a plan for that range of dm_list only."""
         self._h = None
         dm = np.ascontiguousarray(dm_list, dtype=np.float64)
         mask = None if chan_mask is None else np.ascontiguousarray(chan_mask, dtype=np.uint8)
         if mask is not None and mask.shape != (nchan,):
             raise ValueError("chan_mask must have nchan entries")
         h = _vp()
-        code = lib().ddsp_plan_create(ctypes.byref(h), int(nchan), float(f_top_mhz), float(chan_bw_mhz),
-                                      float(tsamp_s), int(nsamp), dm.ctypes.data, int(dm.size),
-                                      int(downsample), mask.ctypes.data if mask is not None else None,
-                                      int(in_dtype))
-        _check(code, "ddsp_plan_create")
+        begin, count = (0, int(dm.size)) if rows is None else (int(rows[0]), int(rows[1]))
+        code = lib().ddsp_plan_create_rows(ctypes.byref(h), int(nchan), float(f_top_mhz), float(chan_bw_mhz),
+                                           float(tsamp_s), int(nsamp), dm.ctypes.data, int(dm.size), begin, count,
+                                           int(downsample), mask.ctypes.data if mask is not None else None,
+                                           int(in_dtype))
+        _check(code, "ddsp_plan_create_rows")
         self._h = h
-        self.nchan, self.ndm, self.nsamp = int(nchan), int(dm.size), int(nsamp)
+        self.nchan, self.ndm, self.nsamp = int(nchan), count, int(nsamp)
         self.downsample, self.in_dtype = int(downsample), int(in_dtype)
         self.in_pitch, self.out_pitch = self.nsamp, self.nsamp_out
 
@@ -209,4 +212,4 @@ def version():
 def plan_for(wl, **kw):
     """Plan for a synth.Workload (argument marshalling only)."""
     return Plan(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.nsamp, wl.dm_list, wl.downsample,
-                wl.mask, DDSP_IN_U8 if wl.dtype == "u8" else DDSP_IN_F32, **kw)
+                wl.mask, DDSP_IN_U8 if wl.dtype == "u8" else DDSP_IN_F32, **kw)   # kw: rows=(begin, count)

@@ -163,18 +163,19 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs
     }
     __syncthreads();
 
-    const int64_t nitems = (int64_t)a.nblk * a.NT;
-    const int64_t first = blockIdx.x, stride = gridDim.x;
-    const int64_t n_my = first < nitems ? (nitems - first + stride - 1) / stride : 0;
-    const int64_t nchunks_my = n_my * a.nchunk;
+    // 32-bit bookkeeping throughout (the plan guarantees nblk * NT * nchunk < 2^31): registers are for accumulators
+    const int nitems = a.nblk * a.NT;
+    const int first = (int)blockIdx.x, stride = (int)gridDim.x;
+    const int n_my = first < nitems ? (nitems - first + stride - 1) / stride : 0;
+    const int nchunks_my = n_my * a.nchunk;
 
     // ---- producer (warp 0): lane r < kC copies row r of a chunk, lane kC copies the chunk's table ----------
-    int64_t p_issued = 0, p_item = first;
+    int p_issued = 0, p_item = first;
     int p_k = 0, p_stage = 0;
     uint32_t p_phase = 0;                                // parity of the use of p_stage that is being filled
     auto issue = [&]() {
-        const int b = (int)(p_item / a.NT);
-        const int64_t tau = p_item - (int64_t)b * a.NT;
+        const int b = p_item / a.NT;
+        const int tau = p_item - b * a.NT;
         const uint32_t st = stages + (uint32_t)p_stage * (uint32_t)a.stage_bytes;
         const uint32_t fb = bar_full + 8 * p_stage;
         if (lane < kC) {
@@ -183,7 +184,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs
             if (l < a.nlist) {
                 const int2 w = __ldg(a.win + (size_t)b * (size_t)(a.nchunk * kC) + l);
                 const int64_t bytes = (int64_t)w.y * K::WB;
-                const int64_t so = ((int64_t)l * a.M + tau * kTW + w.x) * K::WB;
+                const int64_t so = ((int64_t)l * a.M + (int64_t)tau * kTW + w.x) * K::WB;
                 // belt and braces: the plan guarantees all of this; a bad table must not become a bad access
                 if (w.y > 0 && bytes <= a.RS && w.x >= 0 && so >= 0 && so + bytes <= a.y_bytes) {
                     mbar_arrive_expect_tx(fb, (uint32_t)bytes);
@@ -216,10 +217,10 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs
     int c_stage = 0;
     uint32_t c_phase = 0;
     bool aborted = false;
-    for (int64_t it = 0; it < n_my && !aborted; ++it) {
-        const int64_t item = first + it * stride;
-        const int b = (int)(item / a.NT);
-        const int64_t tau = item - (int64_t)b * a.NT;
+    for (int it = 0; it < n_my && !aborted; ++it) {
+        const int item = first + it * stride;
+        const int b = item / a.NT;
+        const int tau = item - b * a.NT;
 #pragma unroll
         for (int j = 0; j < kDT; ++j)
 #pragma unroll
@@ -235,7 +236,7 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs
         // 16-bit lanes -> output rows (uint8 kinds); fp32 accumulators -> output rows (float32, once)
         bool first_flush = true;
         auto flush = [&]() {
-            const int64_t m0 = tau * kTW + slab * (kMW * 32) + lane;        // word of this thread, k = 0
+            const int64_t m0 = (int64_t)tau * kTW + slab * (kMW * 32) + lane;   // word of this thread, k = 0
             const int64_t lim = a.nout - m0;                                   // column k*32 + seg*Q is valid iff < lim
 #pragma unroll
             for (int j = 0; j < kDT; ++j) {
@@ -459,7 +460,7 @@ int ddsp_lanes_plan(ddsp_plan* p) {
         }
     int64_t NT, Q, M;
     ddsp_lanes_range(p, p->nsamp_out, &NT, &Q, &M);
-    if ((int64_t)g.nblk * NT > ((int64_t)1 << 40)) return DDSP_OK;
+    if ((int64_t)g.nblk * NT * std::max(g.nchunk, 1) >= ((int64_t)1 << 31)) return DDSP_OK;   // 32-bit chunk counters
     g.ws_bytes = (size_t)std::max(nlist, 1) * (size_t)M * WB;
     g.ok = true;
     return DDSP_OK;
@@ -534,6 +535,7 @@ cudaError_t ddsp_launch_lanes(const ddsp_plan* p, const void* d_in, void* d_out,
     a.nlist = nlist; a.nchunk = g.nchunk; a.nblk = g.nblk; a.ndm = p->ndm; a.NT = (int)NT; a.RS = g.RS; a.NS = g.NS;
     a.stage_bytes = g.stage_bytes; a.flush_rows = g.flush_rows; a.one = 1u;
     const int64_t nitems = (int64_t)g.nblk * NT;
+    if (nitems * std::max(g.nchunk, 1) >= ((int64_t)1 << 31)) return cudaErrorInvalidConfiguration;
     const unsigned grid = (unsigned)std::min<int64_t>(nitems, p->sm_count > 0 ? p->sm_count : 148);
     kLanesKernels[g.kind]<<<grid, kThreads, g.smem_bytes, s>>>(a);
     return cudaGetLastError();

@@ -60,15 +60,24 @@ const char* ddsp_strerror(int code) {
 int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, double tsamp,
                      int64_t nsamp, const double* dm_list, int ndm, int downsample,
                      const uint8_t* chan_mask, int in_dtype) {
+    return ddsp_plan_create_rows(plan, nchan, f_top, chan_bw, tsamp, nsamp, dm_list, ndm, 0, ndm, downsample,
+                                 chan_mask, in_dtype);
+}
+
+int ddsp_plan_create_rows(ddsp_plan** plan, int nchan, double f_top, double chan_bw, double tsamp,
+                          int64_t nsamp, const double* dm_list, int ndm_all, int row_begin, int row_count,
+                          int downsample, const uint8_t* chan_mask, int in_dtype) {
     if (!plan) return DDSP_ERR_INVALID_ARG;
     *plan = nullptr;
-    if (nchan < 1 || ndm < 1 || downsample < 1 || nsamp < 1 || !dm_list) return DDSP_ERR_INVALID_ARG;
+    if (ndm_all < 1 || row_begin < 0 || row_count < 1 || row_begin > ndm_all - row_count) return DDSP_ERR_INVALID_ARG;
+    const int ndm = row_count;
+    if (nchan < 1 || downsample < 1 || nsamp < 1 || !dm_list) return DDSP_ERR_INVALID_ARG;
     if (!(chan_bw < 0.0) || !(tsamp > 0.0) || !std::isfinite(f_top) || !std::isfinite(chan_bw) ||
         !std::isfinite(tsamp))
         return DDSP_ERR_INVALID_ARG;
     if (!(f_top + (double)(nchan - 1) * chan_bw > 0.0)) return DDSP_ERR_INVALID_ARG;
     if (in_dtype != DDSP_IN_U8 && in_dtype != DDSP_IN_F32) return DDSP_ERR_INVALID_ARG;
-    for (int i = 0; i < ndm; ++i)
+    for (int i = 0; i < ndm_all; ++i)
         if (!std::isfinite(dm_list[i]) || dm_list[i] < 0.0) return DDSP_ERR_INVALID_ARG;
     if ((int64_t)ndm * nchan > ((int64_t)1 << 31) - 1) return DDSP_ERR_UNSUPPORTED;
 
@@ -79,7 +88,7 @@ int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, 
         p->nchan = nchan; p->ndm = ndm; p->ds = downsample; p->in_dtype = in_dtype;
         p->f_top = f_top; p->chan_bw = chan_bw; p->tsamp = tsamp; p->nsamp = nsamp;
         p->nsamp_ds = (nsamp + downsample - 1) / downsample;
-        p->dm.assign(dm_list, dm_list + ndm);
+        p->dm.assign(dm_list + row_begin, dm_list + row_begin + ndm);
         p->mask.assign((size_t)nchan, 0);
         if (chan_mask)
             for (int c = 0; c < nchan; ++c) p->mask[c] = chan_mask[c] ? 1 : 0;
@@ -94,12 +103,16 @@ int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, 
             const double f = f_top + (double)c * chan_bw;
             chan_term[c] = 1.0 / (f * f) - inv_top;
         }
+        // d_max is the maximum over the WHOLE list (all trials, all channels), so that every shard of a list
+        // has the same nsamp_out (invariant I7); only the plan's own rows are kept.
         p->delays.resize((size_t)ndm * nchan);
+        std::vector<int32_t> scratch((size_t)nchan);
         int64_t dmax = 0;
         bool overflow = false;
-        for (int i = 0; i < ndm; ++i) {
+        for (int i = 0; i < ndm_all; ++i) {
             const double kdm = kDispersionConstant * dm_list[i];
-            int32_t* row = &p->delays[(size_t)i * nchan];
+            const bool mine = i >= row_begin && i < row_begin + ndm;
+            int32_t* row = mine ? &p->delays[(size_t)(i - row_begin) * nchan] : scratch.data();
             for (int c = 0; c < nchan; ++c) {
                 const double v = std::floor((kdm * chan_term[c]) / tsamp_ds + 0.5);
                 if (!(v < 2147483647.0)) { overflow = true; break; }
@@ -121,7 +134,7 @@ int ddsp_plan_create(ddsp_plan** plan, int nchan, double f_top, double chan_bw, 
             p->order.resize((size_t)ndm);
             std::iota(p->order.begin(), p->order.end(), 0);
             std::stable_sort(p->order.begin(), p->order.end(),
-                             [&](int a, int b) { return p->dm[a] < p->dm[b]; });
+                             [&](int a, int b) { return p->dm[a] < p->dm[b]; });   // p->dm: the plan's own rows
         }
     } catch (const std::bad_alloc&) {
         rc = DDSP_ERR_ALLOC;

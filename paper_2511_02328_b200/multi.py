@@ -1,8 +1,15 @@
-"""Multi-GPU plumbing: the path shards by independent units with NO data-path
-collective.  A unit is one observation (one filterbank dedispersed over the whole DM grid) -- the way
-the paper runs its four antenna streams side by side -- so every rank owns whole units
-and `torch.distributed` is used only for the barrier around the timed region and for the max-over-
-ranks of the device time.  Works with backend "nccl" (one process per GPU) and "gloo" (CPU tests).
+"""Multi-GPU plumbing.  Two ways to use N GPUs, both without a reduction:
+
+  * independent units (the default of bench.py --gpus N): a unit is one observation dedispersed over the whole
+    DM grid -- the way the paper runs its four antenna streams side by side.  Every rank owns
+    whole units; no collective touches the data.
+  * ONE observation split by DM rows: DM trials are independent, so rank r computes the
+    contiguous row range `shard_rows(ndm, r, world)` with a plan made by ddsp_plan_create_rows (d_max over the
+    whole list, so every shard has the same nsamp_out); the only exchange step is ONE broadcast of the input
+    from the rank that holds it (`broadcast_input`: NCCL over NVLink / NVSwitch on GPUs), outputs stay sharded.
+
+`torch.distributed` also provides the barrier around the timed region and the max-over-ranks of the device
+time.  Works with backend "nccl" (one process per GPU) and "gloo" (CPU tests).
 """
 import os
 
@@ -35,6 +42,21 @@ def shard_units(n_units, rank, world):
     base, rem = divmod(n_units, world)
     lo = rank * base + min(rank, rem)
     return range(lo, lo + base + (1 if rank < rem else 0))
+
+
+def shard_rows(ndm, rank, world):
+    """(row_begin, row_count) of rank `rank` when `ndm` DM rows are split into contiguous, balanced ranges
+    (row_count may be 0 when there are more ranks than rows)."""
+    r = shard_units(ndm, rank, world)
+    return r.start, len(r)
+
+
+def broadcast_input(x, src=0):
+    """The one exchange step of the DM-row split: the filterbank of rank `src` is copied into every rank's `x`
+    (same shape and dtype everywhere), in place.  NCCL for CUDA tensors, gloo for CPU tensors."""
+    if dist.is_initialized() and dist.get_world_size() > 1:
+        dist.broadcast(x, src=src)
+    return x
 
 
 def barrier():

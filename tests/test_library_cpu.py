@@ -132,3 +132,18 @@ def test_product_does_not_import_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), f
                 assert "oracle_ddsp" not in text and "liboracle" not in text, f
+
+
+def test_plan_rows_is_a_row_range_of_the_whole_plan(lib, oracle):
+    """ddsp_plan_create_rows: the delay table is the row range, d_max and nsamp_out are the whole
+    list's (invariant I7), whatever the range."""
+    wl = synth.config("tiny")
+    want, dmax = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, 1)
+    for begin, count in ((0, 201), (0, 50), (50, 100), (200, 1), (13, 16)):
+        with binding.plan_for(wl, rows=(begin, count)) as plan:
+            assert plan.ndm == count
+            assert np.array_equal(plan.get_delays(), want[begin:begin + count])
+            assert plan.max_delay == dmax and plan.nsamp_out == wl.nsamp - dmax
+    for bad in ((-1, 5), (0, 0), (200, 2), (201, 1)):
+        with pytest.raises(binding.DdspError):
+            binding.plan_for(wl, rows=bad)
