@@ -130,6 +130,16 @@ DDSP_API int ddsp_execute_ws(const ddsp_plan* plan, const void* d_in, void* d_ou
  * h_out: ndm rows of out_pitch elements.  Not re-entrant for one plan (the staging buffers are shared). */
 DDSP_API int ddsp_execute_host(ddsp_plan* plan, const void* h_in, void* h_out, void* cuda_stream);
 
+/* ddsp_execute_host with the three phases overlapped (the paper names the copies, not the kernel, as its
+ * bottleneck and leaves their overlap undone): the output columns are cut into
+ * npieces runs; run j needs input columns < (end_j + d_max) * ds only, so the copy of the input for run j+1, the
+ * kernels of run j and the copy of run j-1's result proceed at the same time on three internal streams.  Same
+ * buffers, layout and result as ddsp_execute_host; synchronises cuda_stream first and returns when everything
+ * is done.  Pinned host memory is needed for real overlap.  DDSP_ERR_UNSUPPORTED unless the plan's kernel is
+ * DDSP_KERNEL_LANES (the kernels that can be launched on a run of output columns). */
+DDSP_API int ddsp_execute_host_pipelined(ddsp_plan* plan, const void* h_in, void* h_out, void* cuda_stream,
+                                         int npieces);
+
 DDSP_API int ddsp_plan_destroy(ddsp_plan* plan); /* NULL is allowed */
 
 DDSP_API const char* ddsp_strerror(int code);

@@ -35,6 +35,7 @@ SIGNATURES = {
     "ddsp_execute": (_i, [_vp, _vp, _vp, _vp]),
     "ddsp_execute_ws": (_i, [_vp, _vp, _vp, _vp, _i64, _vp]),
     "ddsp_execute_host": (_i, [_vp, _vp, _vp, _vp]),
+    "ddsp_execute_host_pipelined": (_i, [_vp, _vp, _vp, _vp, _i]),
     "ddsp_plan_destroy": (_i, [_vp]),
     "ddsp_strerror": (_cp, [_i]),
     "ddsp_last_cuda_error": (_i, [_vp]),
@@ -168,6 +169,17 @@ class Plan:
         s = torch.cuda.current_stream() if stream is None else stream
         _check(lib().ddsp_execute_host(self._h, _vp(xp), _vp(op), _vp(s.cuda_stream)),
                "ddsp_execute_host", self._h)
+        return out
+
+    def execute_host_pipelined(self, x, out, stream=None, npieces=8):
+        """ddsp_execute_host_pipelined: copies and kernels overlapped over `npieces` runs of output columns."""
+        import torch
+        self._check_buffers(x, out, cuda=False)
+        xp = x.data_ptr() if hasattr(x, "data_ptr") else x.ctypes.data
+        op = out.data_ptr() if hasattr(out, "data_ptr") else out.ctypes.data
+        s = torch.cuda.current_stream() if stream is None else stream
+        _check(lib().ddsp_execute_host_pipelined(self._h, _vp(xp), _vp(op), _vp(s.cuda_stream), int(npieces)),
+               "ddsp_execute_host_pipelined", self._h)
         return out
 
     def _check_buffers(self, x, out, cuda):

@@ -83,6 +83,8 @@ struct ddsp_plan {
     // staging buffers of ddsp_execute_host
     void* d_stage_in = nullptr;
     void* d_stage_out = nullptr;
+    // streams of ddsp_execute_host_pipelined (created on first use)
+    cudaStream_t hs_in = nullptr, hs_k = nullptr, hs_out = nullptr;
 };
 
 // ddsp_direct.cu

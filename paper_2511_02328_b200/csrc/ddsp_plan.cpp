@@ -276,6 +276,59 @@ int ddsp_execute_host(ddsp_plan* p, const void* h_in, void* h_out, void* cuda_st
     return note_cuda(p, e);
 }
 
+int ddsp_execute_host_pipelined(ddsp_plan* p, const void* h_in, void* h_out, void* cuda_stream, int npieces) {
+    if (!p || !h_in || !h_out || npieces < 1) return DDSP_ERR_INVALID_ARG;
+    if (p->device < 0) return DDSP_ERR_CUDA;
+    // only the lanes kernels can be launched on a range of output columns
+    if (p->kernel != DDSP_KERNEL_LANES || !p->lanes.ok) return DDSP_ERR_UNSUPPORTED;
+    const size_t esize = elem_size_in(p);
+    const size_t in_bytes = (size_t)p->nchan * (size_t)p->in_pitch * esize;
+    const size_t out_bytes = (size_t)p->ndm * (size_t)p->out_pitch * 4;
+    cudaError_t e = cudaSuccess;
+    if (!p->d_stage_in) e = cudaMalloc(&p->d_stage_in, in_bytes);
+    if (e == cudaSuccess && !p->d_stage_out) e = cudaMalloc(&p->d_stage_out, out_bytes);
+    if (e == cudaSuccess && !p->hs_in) e = cudaStreamCreateWithFlags(&p->hs_in, cudaStreamNonBlocking);
+    if (e == cudaSuccess && !p->hs_k) e = cudaStreamCreateWithFlags(&p->hs_k, cudaStreamNonBlocking);
+    if (e == cudaSuccess && !p->hs_out) e = cudaStreamCreateWithFlags(&p->hs_out, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)cuda_stream);   // work queued before this call
+    if (e != cudaSuccess) return note_cuda(p, e);
+
+    const int64_t nout = p->nsamp_out;
+    const int64_t piece = (nout + npieces - 1) / npieces;
+    const size_t in_pitch_b = (size_t)p->in_pitch * esize, out_pitch_b = (size_t)p->out_pitch * 4;
+    std::vector<cudaEvent_t> events;
+    int64_t in_done = 0;      // native input columns [0, in_done) are on the device (or on their way, in order)
+    for (int64_t a = 0; a < nout && e == cudaSuccess; a += piece) {
+        const int64_t b = std::min(a + piece, nout);
+        // outputs [a, b) read downsampled samples < b + d_max, i.e. native columns < (b + d_max) * ds
+        const int64_t need = std::min<int64_t>(p->nsamp, (b + p->dmax) * p->ds);
+        cudaEvent_t ev_in = nullptr, ev_k = nullptr;
+        e = cudaEventCreateWithFlags(&ev_in, cudaEventDisableTiming);
+        if (e == cudaSuccess) { events.push_back(ev_in); e = cudaEventCreateWithFlags(&ev_k, cudaEventDisableTiming); }
+        if (e == cudaSuccess) events.push_back(ev_k);
+        if (e == cudaSuccess && need > in_done) {
+            e = cudaMemcpy2DAsync((char*)p->d_stage_in + (size_t)in_done * esize, in_pitch_b,
+                                  (const char*)h_in + (size_t)in_done * esize, in_pitch_b,
+                                  (size_t)(need - in_done) * esize, (size_t)p->nchan, cudaMemcpyHostToDevice, p->hs_in);
+            in_done = need;
+        }
+        if (e == cudaSuccess) e = cudaEventRecord(ev_in, p->hs_in);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->hs_k, ev_in, 0);
+        // the pieces share the plan's workspace: they are ordered on one stream
+        if (e == cudaSuccess) e = ddsp_launch_lanes(p, p->d_stage_in, p->d_stage_out, nullptr, p->hs_k, a, b - a);
+        if (e == cudaSuccess) e = cudaEventRecord(ev_k, p->hs_k);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(p->hs_out, ev_k, 0);
+        if (e == cudaSuccess)
+            e = cudaMemcpy2DAsync((char*)h_out + (size_t)a * 4, out_pitch_b, (const char*)p->d_stage_out + (size_t)a * 4,
+                                  out_pitch_b, (size_t)(b - a) * 4, (size_t)p->ndm, cudaMemcpyDeviceToHost, p->hs_out);
+    }
+    // drain everything that was enqueued, also after an error
+    cudaError_t e1 = cudaStreamSynchronize(p->hs_in), e2 = cudaStreamSynchronize(p->hs_k), e3 = cudaStreamSynchronize(p->hs_out);
+    for (cudaEvent_t ev : events) cudaEventDestroy(ev);
+    if (e == cudaSuccess) e = e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3);
+    return note_cuda(p, e);
+}
+
 int ddsp_plan_destroy(ddsp_plan* p) {
     if (!p) return DDSP_OK;
     ddsp_tiled_free(p);
@@ -284,6 +337,9 @@ int ddsp_plan_destroy(ddsp_plan* p) {
     if (p->d_chan_list) cudaFree(p->d_chan_list);
     if (p->d_stage_in) cudaFree(p->d_stage_in);
     if (p->d_stage_out) cudaFree(p->d_stage_out);
+    if (p->hs_in) cudaStreamDestroy(p->hs_in);
+    if (p->hs_k) cudaStreamDestroy(p->hs_k);
+    if (p->hs_out) cudaStreamDestroy(p->hs_out);
     delete p;
     return DDSP_OK;
 }

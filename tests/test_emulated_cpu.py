@@ -64,7 +64,7 @@ class DeviceArray:
         self._emu.ddsp_emu_unregister(self.a.ctypes.data)
 
 
-def run_emulated(emu, wl, x, in_pitch, kernel, out_extra=3, misalign=0, expect_faults=False):
+def run_emulated(emu, wl, x, in_pitch, kernel, out_extra=3, misalign=0, expect_faults=False, host_pieces=0):
     dm = np.ascontiguousarray(wl.dm_list, dtype=np.float64)
     mask = None if wl.mask is None else np.ascontiguousarray(wl.mask, dtype=np.uint8)
     h = ctypes.c_void_p()
@@ -85,7 +85,10 @@ def run_emulated(emu, wl, x, in_pitch, kernel, out_extra=3, misalign=0, expect_f
         xin.a[...] = x
         out = DeviceArray(emu, (wl.ndm, out_pitch), np.uint32 if wl.dtype == "u8" else np.float32, fill=7)
         f0 = emu.ddsp_emu_faults()
-        rc = emu.ddsp_execute(h, xin.a.ctypes.data, out.a.ctypes.data, None)
+        if host_pieces:     # overlapped host-buffer path: the plan's own staging buffers, runs of output columns
+            rc = emu.ddsp_execute_host_pipelined(h, xin.a.ctypes.data, out.a.ctypes.data, None, host_pieces)
+        else:
+            rc = emu.ddsp_execute(h, xin.a.ctypes.data, out.a.ctypes.data, None)
         assert rc == 0, rc
         st = ctypes.c_int(-1)
         assert emu.ddsp_plan_device_status(h, ctypes.byref(st)) == 0
@@ -109,10 +112,10 @@ def host_input(wl, pitch=None):
     return synth.make_input(wl, "cpu", pitch=pitch).numpy()
 
 
-def check(emu, oracle, wl, kernel, pitch=None, misalign=0):
+def check(emu, oracle, wl, kernel, pitch=None, misalign=0, host_pieces=0):
     pitch = wl.nsamp if pitch is None else pitch
     x = host_input(wl, pitch)
-    got, nout = run_emulated(emu, wl, x, pitch, kernel, misalign=misalign)
+    got, nout = run_emulated(emu, wl, x, pitch, kernel, misalign=misalign, host_pieces=host_pieces)
     want, nout_o, _ = oracle.dedisperse(x, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, nsamp=wl.nsamp,
                                         downsample=wl.downsample, mask=wl.mask)
     assert nout == nout_o
@@ -214,6 +217,20 @@ def test_lanes_real_geometries_cropped(emu, oracle, name, extra):
     _, dmax = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, wl.downsample)
     wl = wl.cropped(wl.downsample * (dmax + extra) - (1 if wl.downsample > 1 else 0))
     check(emu, oracle, wl, LANES)
+
+
+@pytest.mark.parametrize("kind,pieces", [("u8", 3), ("u8", 7), ("bins4", 3), ("f32", 2)])
+def test_lanes_host_pipelined_runs(emu, oracle, kind, pieces):
+    """ddsp_execute_host_pipelined: each run of output columns is its own interleave + accumulate launch pair (own
+    segment length Q, own tiles) after only the input columns it needs (< (end + d_max) * ds) were copied; the
+    runs do not divide the output evenly; the result equals the oracle."""
+    if kind == "u8":
+        wl = small(nsamp=2600, dm_max=50.0, mask_frac=0.1)
+    elif kind == "bins4":
+        wl = small(ds=4, nsamp=4 * 2100 + 2, dm_max=120.0)
+    else:
+        wl = small(dtype="f32", nsamp=1900, dm_max=40.0)
+    check(emu, oracle, wl, LANES, host_pieces=pieces)
 
 
 # ---- the checks can fail: negative controls -------------------------------------------------------------------

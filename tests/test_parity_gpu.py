@@ -258,6 +258,42 @@ def test_execute_host_matches_device(oracle):
         assert np.array_equal(oh.numpy().view(np.uint32), dev)
 
 
+@pytest.mark.parametrize("npieces", [1, 3, 8])
+def test_execute_host_pipelined_lanes(oracle, npieces):
+    """Overlapped host-buffer execute (lanes kernels): same result as the oracle, whatever the number of runs."""
+    wl = _small(nsamp=9000)
+    x = make_input(oracle, wl, "cuda")
+    with binding.plan_for(wl) as plan:
+        _set_kernel(plan, binding.DDSP_KERNEL_LANES)
+        xh = x.cpu().pin_memory()
+        oh = torch.full((plan.ndm, plan.out_pitch), -5, dtype=torch.int32).pin_memory()
+        plan.execute_host_pipelined(xh, oh, npieces=npieces)
+        assert plan.device_status() == 0
+        want, _, _ = oracle.dedisperse(xh.numpy(), wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list)
+        assert_u32_equal(oh.numpy().view(np.uint32)[:, :plan.nsamp_out], want, "pipelined")
+
+
+def test_lanes_two_streams_own_workspaces(oracle):
+    """Two executes of ONE lanes plan that overlap in time: each brings its own workspace (ddsp_execute_ws)."""
+    wl = _small(nsamp=7000)
+    x1 = make_input(oracle, wl, "cuda")
+    x2 = torch.flip(x1, dims=[1]).contiguous()
+    with binding.plan_for(wl) as plan:
+        _set_kernel(plan, binding.DDSP_KERNEL_LANES)
+        ws = [torch.empty(plan.workspace_bytes, dtype=torch.uint8, device="cuda") for _ in range(2)]
+        o1 = torch.empty((plan.ndm, plan.out_pitch), dtype=torch.int32, device="cuda")
+        o2 = torch.empty_like(o1)
+        s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        plan.execute(x1, o1, stream=s1, workspace=ws[0])
+        plan.execute(x2, o2, stream=s2, workspace=ws[1])
+        torch.cuda.synchronize()
+        assert plan.device_status() == 0
+        for xx, oo in ((x1, o1), (x2, o2)):
+            want, _, _ = oracle.dedisperse(xx.cpu().numpy(), wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list)
+            assert_u32_equal(to_host(oo, plan), want, "stream")
+
+
 def test_two_streams_concurrent(oracle):
     wl = _small(nsamp=7000)
     x1 = make_input(oracle, wl, "cuda")
