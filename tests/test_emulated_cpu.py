@@ -307,3 +307,34 @@ def test_lanes_race_check_can_fail():
                                               "ddsp_lanes.cu"))
     r = _run_tsan(exe, "u8", halt=1)          # the first report ends the run
     assert "ThreadSanitizer: data race" in r.stderr
+
+
+# ---- seeded random plans: whatever the shape, the lanes kernels equal the oracle and stay inside their buffers -----
+def test_lanes_random_plans(emu, oracle):
+    rng = np.random.default_rng(20261105)
+    done = 0
+    for trial in range(40):
+        dtype = "f32" if rng.random() < 0.3 else "u8"
+        ds = int(rng.choice([1, 1, 2, 3, 4, 5, 7, 16]))
+        nchan = int(rng.integers(1, 34))
+        ndm = int(rng.integers(1, 40))
+        f_top = float(rng.choice([1500.0, 800.0, 400.0]))
+        wl = synth.Workload("rnd", int(rng.integers(0, 1000)), nchan, f_top, -float(rng.uniform(0.5, 8.0)),
+                            float(rng.choice([1e-3, 2.5e-4])), 1, np.sort(rng.uniform(0.0, 40.0 * ds, ndm)),
+                            downsample=ds, dtype=dtype, mean=128.0 if dtype == "u8" else 0.0,
+                            std=50.0 if dtype == "u8" else 1.0)
+        if rng.random() < 0.5:
+            wl.mask = (rng.random(nchan) < 0.3).astype(np.uint8)
+        if rng.random() < 0.3:
+            wl.dm_list = rng.permutation(wl.dm_list)
+        _, dmax = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, ds)
+        if dmax > 3000:
+            continue
+        nout = int(rng.integers(1, 1400))
+        wl = wl.cropped(ds * (dmax + nout) - int(rng.integers(0, ds)))
+        pitch = wl.nsamp + int(rng.integers(0, 20))
+        check(emu, oracle, wl, LANES, pitch=pitch, misalign=int(rng.integers(0, 4)) * (4 if dtype == "f32" else 1))
+        done += 1
+        if done == 12:
+            break
+    assert done == 12
