@@ -24,6 +24,17 @@ DDSP_API int ddsp_testing_lanes_geometry(const ddsp_plan* plan, int64_t* geom);
  * rows: host int32[blocks * trials per block] output row of each DM-sorted trial, -1 = padding. */
 DDSP_API int ddsp_testing_lanes_tables(const ddsp_plan* plan, int32_t* win, uint32_t* off, int32_t* rows);
 
+/* Tiled kernel (uint8, ds = 1).  geom: host int64[10] = {trials per block, output samples
+ * per tile T, DM blocks, time tiles, rows per chunk, stages, row stride (bytes of one phase copy), shared memory
+ * bytes, chunks, padded channel count}.
+ * base: int32[blocks * padded channels] 16-byte-aligned first delay of the block per listed channel;
+ * nunit: int32[same] 16-byte units of the row window that are staged; chan: int32[padded channels] channel of
+ * each listed entry (padding repeats the last); off: uint32[blocks * padded channels * trials per block]
+ * stage-relative byte offset ((slot * 4 + phase) * row stride + word * 4); rows: int32[blocks * trials per block]. */
+DDSP_API int ddsp_testing_tiled_geometry(const ddsp_plan* plan, int64_t* geom);
+DDSP_API int ddsp_testing_tiled_tables(const ddsp_plan* plan, int32_t* base, int32_t* nunit, int32_t* chan, uint32_t* off,
+                                       int32_t* rows);
+
 #ifdef __cplusplus
 }
 #endif

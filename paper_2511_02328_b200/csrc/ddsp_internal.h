@@ -33,6 +33,10 @@ struct ddsp_tiled {
     std::vector<int32_t> h_base;  // [nblk][nch_pad] 16-byte-aligned first delay of the block per listed channel
     std::vector<uint16_t> h_nunit; // [nblk][nch_pad] 16-byte units of each row window that are needed
     std::vector<int32_t> h_chan;  // [nch_pad] channel index of each listed channel (padding repeats the last)
+#ifdef DDSP_TESTING
+    std::vector<uint32_t> h_off;  // host copies of d_off / d_rows for the table tests (include/ddsp_testing.h)
+    std::vector<int32_t> h_rows;
+#endif
     int nch_pad = 0;              // nchan_unmasked rounded up to chunk_c
 };
 

@@ -364,6 +364,10 @@ static int tiled_build_tables(ddsp_plan* p) {
             g.h_nunit[(size_t)b * g.nch_pad + l] = (uint16_t)(l < nlist ? std::min(need, g.row_stride / 16) : 0);
         }
     }
+#ifdef DDSP_TESTING
+    g.h_off = off;
+    g.h_rows = rows;
+#endif
     if (p->device < 0) return DDSP_OK;   // host-only plan: geometry only
     cudaError_t e = upload(&g.d_off, off);
     if (e == cudaSuccess) e = upload(&g.d_rows, rows);
@@ -436,3 +440,32 @@ cudaError_t ddsp_launch_tiled(const ddsp_plan* p, const void* d_in, void* d_out,
     kVariants[g.variant].fn<<<grid, g.threads, g.smem_bytes, s>>>(a);
     return cudaGetLastError();
 }
+
+#ifdef DDSP_TESTING
+// Introspection for the CPU tests (include/ddsp_testing.h); not part of the product library.
+#include "../../include/ddsp_testing.h"
+#include <cstring>
+
+extern "C" int ddsp_testing_tiled_geometry(const ddsp_plan* p, int64_t* geom) {
+    if (!p || !geom) return DDSP_ERR_INVALID_ARG;
+    const ddsp_tiled& g = p->tiled;
+    if (!g.ok) return DDSP_ERR_UNSUPPORTED;
+    const int64_t v[10] = {g.bdm, g.tile_t, g.nblk, g.ntile_t, g.chunk_c, g.nstage, g.row_stride, g.smem_bytes, g.nchunk,
+                           g.nch_pad};
+    std::memcpy(geom, v, sizeof(v));
+    return DDSP_OK;
+}
+
+extern "C" int ddsp_testing_tiled_tables(const ddsp_plan* p, int32_t* base, int32_t* nunit, int32_t* chan, uint32_t* off,
+                                         int32_t* rows) {
+    if (!p || !base || !nunit || !chan || !off || !rows) return DDSP_ERR_INVALID_ARG;
+    const ddsp_tiled& g = p->tiled;
+    if (!g.ok) return DDSP_ERR_UNSUPPORTED;
+    std::memcpy(base, g.h_base.data(), g.h_base.size() * sizeof(int32_t));
+    for (size_t i = 0; i < g.h_nunit.size(); ++i) nunit[i] = g.h_nunit[i];
+    std::memcpy(chan, g.h_chan.data(), g.h_chan.size() * sizeof(int32_t));
+    std::memcpy(off, g.h_off.data(), g.h_off.size() * sizeof(uint32_t));
+    std::memcpy(rows, g.h_rows.data(), g.h_rows.size() * sizeof(int32_t));
+    return DDSP_OK;
+}
+#endif  // DDSP_TESTING
