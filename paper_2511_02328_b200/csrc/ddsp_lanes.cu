@@ -34,6 +34,7 @@
 // with a reduction store (RED, no return value, nobody waits).  Every output element is owned by one thread.
 #include <algorithm>
 #include <climits>
+#include <type_traits>
 #include <vector>
 
 #include "ddsp_internal.h"
@@ -234,69 +235,92 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs
                 }
 
         // 16-bit lanes -> output rows (uint8 kinds); fp32 accumulators -> output rows (float32, once)
+        // 16-bit lanes -> uint32 output rows (first flush of the item: store; later: reduction); fp32 accumulators ->
+        // output rows, once.  Column offsets are 32-bit (W * Q < 2^31, checked at launch).  The common case -- a real
+        // trial, every column of this thread inside [0, nout) -- runs without a per-element test.
         bool first_flush = true;
-        auto flush = [&]() {
+        // FIRST: plain stores, else reductions; CHECKED: test every column against the end of the output
+        auto flush_body = [&](auto first_tag, auto checked_tag) {
+            constexpr bool FIRST = decltype(first_tag)::value, CHECKED = decltype(checked_tag)::value;
             const int64_t m0 = (int64_t)tau * kTW + slab * (kMW * 32) + lane;   // word of this thread, k = 0
-            const int64_t lim = a.nout - m0;                                   // column k*32 + seg*Q is valid iff < lim
+            const int64_t lim64 = a.nout - m0;                                  // column offset c is valid iff c < lim
+            const uint32_t lim = lim64 <= 0 ? 0u : (lim64 > 0x7fffffffLL ? 0x7fffffffu : (uint32_t)lim64);
+            const uint32_t q32 = (uint32_t)a.Q;
+            auto emit = [&](char* base, uint32_t col, uint32_t v) {
+                if (CHECKED && col >= lim) return;
+                uint32_t* p = reinterpret_cast<uint32_t*>(base + (size_t)col * 4u);     // col is warp-uniform
+                if (FIRST) st_global_u32(p, v);
+                else red_add_u32(p, v);
+            };
 #pragma unroll
             for (int j = 0; j < kDT; ++j) {
                 int row = __ldg(a.rows + b * kBDM + grp * kDT + j);
                 if (row >= a.ndm) row = -1;
-                const int64_t obase = (int64_t)row * a.out_pitch + a.u_begin + m0;
+                char* const base = (char*)a.out + ((int64_t)(row < 0 ? 0 : row) * a.out_pitch + a.u_begin + m0) * 4;
+                const bool live = row >= 0 && lim > 0u;
 #pragma unroll
                 for (int k = 0; k < kMW; ++k) {
 #pragma unroll
                     for (int h = 0; h < K::NR; ++h) {
                         if constexpr (KIND == kKindF32) {
-                            const int64_t col = (int64_t)h * a.Q + k * 32;
-                            if (row >= 0 && col < lim) st_global_f32((float*)a.out + obase + col, accf[j][k][h]);
-                        } else {
-                            uint32_t v[4];
-                            int nv;
-                            int64_t seg0;
-                            if constexpr (KIND == kKindU8) {       // (b0, b1, b2, b3) of the half word = segments 4h .. 4h+3
-                                const uint32_t o = acc[j][k][h][kNAcc - 1];
-                                const uint32_t e = acc[j][k][h][0] - (o << 8);     // exact mod 2^32
-                                v[0] = e & 0xffffu; v[1] = o & 0xffffu; v[2] = e >> 16; v[3] = o >> 16;
-                                nv = 4; seg0 = 4 * h;
-                            } else {                      // two 16-bit bins = segments 2h, 2h+1
-                                const uint32_t s = acc[j][k][h][0];
-                                v[0] = s & 0xffffu; v[1] = s >> 16; v[2] = 0; v[3] = 0;
-                                nv = 2; seg0 = 2 * h;
+                            const uint32_t col = (uint32_t)h * q32 + (uint32_t)(k * 32);
+                            if (live && (!CHECKED || col < lim))
+                                st_global_f32(reinterpret_cast<float*>(base + (size_t)col * 4u), accf[j][k][h]);
+                        } else if constexpr (KIND == kKindU8) {   // (b0, b1, b2, b3) of the half word = segments 4h .. 4h+3
+                            const uint32_t o = acc[j][k][h][1];
+                            const uint32_t e = acc[j][k][h][0] - (o << 8);      // exact mod 2^32
+                            acc[j][k][h][0] = 0u; acc[j][k][h][1] = 0u;
+                            if (live) {
+                                const uint32_t c0 = (uint32_t)(4 * h) * q32 + (uint32_t)(k * 32);
+                                emit(base, c0, e & 0xffffu);
+                                emit(base, c0 + q32, o & 0xffffu);
+                                emit(base, c0 + 2u * q32, e >> 16);
+                                emit(base, c0 + 3u * q32, o >> 16);
                             }
-#pragma unroll
-                            for (int e = 0; e < kNAcc; ++e) acc[j][k][h][e] = 0u;
-#pragma unroll
-                            for (int s = 0; s < 4; ++s) {
-                                if (s >= nv) continue;
-                                const int64_t col = (seg0 + s) * a.Q + k * 32;
-                                if (row >= 0 && col < lim) {
-                                    uint32_t* p = (uint32_t*)a.out + obase + col;
-                                    if (first_flush) st_global_u32(p, v[s]);
-                                    else red_add_u32(p, v[s]);
-                                }
+                        } else {                                   // two 16-bit bins = segments 2h, 2h+1
+                            const uint32_t sum = acc[j][k][h][0];
+                            acc[j][k][h][0] = 0u;
+                            if (live) {
+                                const uint32_t c0 = (uint32_t)(2 * h) * q32 + (uint32_t)(k * 32);
+                                emit(base, c0, sum & 0xffffu);
+                                emit(base, c0 + q32, sum >> 16);
                             }
                         }
                     }
                 }
             }
+        };
+        // 16-bit lanes -> uint32 output rows (first flush of the item: store; later: reduction); fp32 accumulators ->
+        // output rows, once.  Column offsets are 32-bit (W * Q < 2^31, checked at launch).  The common case -- every
+        // column of this thread inside [0, nout) -- runs without a per-element test.
+        auto flush = [&]() {
+            const int64_t lim64 = a.nout - ((int64_t)tau * kTW + slab * (kMW * 32) + lane);
+            const bool all_cols = (int64_t)(K::W - 1) * a.Q + (kMW - 1) * 32 < lim64;
+            if (first_flush) {
+                if (all_cols) flush_body(std::true_type{}, std::false_type{});
+                else flush_body(std::true_type{}, std::true_type{});
+            } else {
+                if (all_cols) flush_body(std::false_type{}, std::false_type{});
+                else flush_body(std::false_type{}, std::true_type{});
+            }
             first_flush = false;
         };
 
         int since_flush = 0;
-        for (int k_chunk = 0; k_chunk < a.nchunk; ++k_chunk) {
-            // producer: refill the stage that every warp left two chunks ago
-            if (warp == 0 && p_issued < nchunks_my) {
+        for (int k_chunk = 0;; ++k_chunk) {
+            const bool last = k_chunk == a.nchunk;
+            // producer: refill the stage that every warp left two chunks ago (also while this warp flushes)
+            if (!last && warp == 0 && p_issued < nchunks_my) {
                 bool ok = true;
                 if (p_issued >= a.NS) ok = mbar_wait(bar_empty + 8 * p_stage, p_phase ^ 1u, abort_flag, a.wait_budget);
                 if (ok) issue();
                 else { aborted = true; break; }
             }
-            if (!mbar_wait(bar_full + 8 * c_stage, c_phase, abort_flag, a.wait_budget)) { aborted = true; break; }
-
-            const int nrow = min(kC, a.nlist - k_chunk * kC);
-            if (KIND != kKindF32 && since_flush + nrow > a.flush_rows) { flush(); since_flush = 0; }
+            const int nrow = last ? 0 : min(kC, a.nlist - k_chunk * kC);
+            if (last || (KIND != kKindF32 && since_flush + nrow > a.flush_rows)) { flush(); since_flush = 0; }   // the one call site
+            if (last) break;
             since_flush += nrow;
+            if (!mbar_wait(bar_full + 8 * c_stage, c_phase, abort_flag, a.wait_budget)) { aborted = true; break; }
 
             const uint32_t st = stages + (uint32_t)c_stage * (uint32_t)a.stage_bytes;
             const uint32_t tptr = st + (uint32_t)(kC * a.RS) + (uint32_t)(grp * (kDT * 4));
@@ -363,7 +387,6 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs
             if (lane == 0) mbar_arrive(bar_empty + 8 * c_stage);     // this warp is done with the stage
             if (++c_stage == a.NS) { c_stage = 0; c_phase ^= 1u; }
         }
-        if (!aborted) flush();
     }
     if (aborted) report_status(a.status, kStatusTimeout);
 }
@@ -536,6 +559,7 @@ cudaError_t ddsp_launch_lanes(const ddsp_plan* p, const void* d_in, void* d_out,
     a.stage_bytes = g.stage_bytes; a.flush_rows = g.flush_rows; a.one = 1u;
     const int64_t nitems = (int64_t)g.nblk * NT;
     if (nitems * std::max(g.nchunk, 1) >= ((int64_t)1 << 31)) return cudaErrorInvalidConfiguration;
+    if (Q * kLanesPerWord[g.kind] >= ((int64_t)1 << 31)) return cudaErrorInvalidConfiguration;      // 32-bit column offsets
     const unsigned grid = (unsigned)std::min<int64_t>(nitems, p->sm_count > 0 ? p->sm_count : 148);
     kLanesKernels[g.kind]<<<grid, kThreads, g.smem_bytes, s>>>(a);
     return cudaGetLastError();

@@ -35,17 +35,6 @@ def crop(oracle, wl, extra_out):
     return wl.cropped(wl.downsample * (dmax + int(extra_out)))
 
 
-def sample_rows(ndm, nrows, seed=0, always=()):
-    """Sorted unique row indices: first, last, `always`, block edges and a seeded random fill."""
-    rng = np.random.default_rng(seed)
-    rows = {0, ndm - 1}
-    rows.update(int(r) for r in always if 0 <= int(r) < ndm)
-    for b in (8, 16, 32):
-        for k in (1, ndm // (2 * b)):
-            rows.update(r for r in (k * b - 1, k * b) if 0 <= r < ndm)
-    while len(rows) < min(nrows, ndm):
-        rows.add(int(rng.integers(0, ndm)))
-    return np.array(sorted(rows), dtype=np.int64)
 
 
 def assert_u32_equal(got, want, what=""):
