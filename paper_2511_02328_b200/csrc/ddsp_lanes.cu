@@ -147,6 +147,7 @@ template <int KIND, int FMA_E>
 __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs a) {
     using K = Kind<KIND>;
     constexpr int kNAcc = KIND == kKindU8 ? 2 : 1;      // accumulator registers per loaded register
+    constexpr int kLB = K::NR == 2 ? 4 : 2;             // words per row loaded before their adds are issued
     extern __shared__ __align__(128) uint8_t smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int slab = warp % kSlabs, grp = warp / kSlabs;
@@ -333,26 +334,40 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs
 #pragma unroll
                 for (int j = 0; j < kDT; ++j) {
                     const uint32_t a0 = rb + o0[j], a1 = rb + o1[j];
+                    // loads of a batch of words first (kLB x 2 rows in flight per thread), then their adds: the
+                    // shared-memory pipe stays full from 16 warps (Little's law), not from long dependency chains
 #pragma unroll
-                    for (int k = 0; k < kMW; ++k) {
-                        uint32_t w0[K::NR], w1[K::NR];
-                        if constexpr (K::NR == 2) { lds64(a0 + k * 32 * K::WB, w0); lds64(a1 + k * 32 * K::WB, w1); }
-                        else { lds128(a0 + k * 32 * K::WB, w0); lds128(a1 + k * 32 * K::WB, w1); }
+                    for (int kb = 0; kb < kMW; kb += kLB) {
+                        uint32_t w0[kLB][K::NR], w1[kLB][K::NR];
 #pragma unroll
-                        for (int h = 0; h < K::NR; ++h) {
-                            if constexpr (KIND == kKindU8) {
-                                if constexpr (FMA_E != 0) {
-                                    add_fma_pipe(acc[j][k][h][0], w0[h], one);
-                                    add_fma_pipe(acc[j][k][h][0], w1[h], one);
-                                } else {
-                                    acc[j][k][h][0] = acc[j][k][h][0] + w0[h] + w1[h];
+                        for (int q = 0; q < kLB; ++q) {
+                            if constexpr (K::NR == 2) lds64(a0 + (kb + q) * 32 * K::WB, w0[q]);
+                            else lds128(a0 + (kb + q) * 32 * K::WB, w0[q]);
+                        }
+#pragma unroll
+                        for (int q = 0; q < kLB; ++q) {
+                            if constexpr (K::NR == 2) lds64(a1 + (kb + q) * 32 * K::WB, w1[q]);
+                            else lds128(a1 + (kb + q) * 32 * K::WB, w1[q]);
+                        }
+#pragma unroll
+                        for (int q = 0; q < kLB; ++q) {
+                            const int k = kb + q;
+#pragma unroll
+                            for (int h = 0; h < K::NR; ++h) {
+                                if constexpr (KIND == kKindU8) {
+                                    if constexpr (FMA_E != 0) {
+                                        add_fma_pipe(acc[j][k][h][0], w0[q][h], one);
+                                        add_fma_pipe(acc[j][k][h][0], w1[q][h], one);
+                                    } else {
+                                        acc[j][k][h][0] = acc[j][k][h][0] + w0[q][h] + w1[q][h];
+                                    }
+                                    acc[j][k][h][kNAcc - 1] = acc[j][k][h][kNAcc - 1] + odd_bytes(w0[q][h]) + odd_bytes(w1[q][h]);
+                                } else if constexpr (KIND == kKindU16) {
+                                    acc[j][k][h][0] = acc[j][k][h][0] + w0[q][h] + w1[q][h];
+                                } else {                  // ascending channel order, one rounding per add
+                                    accf[j][k][h] = __fadd_rn(__fadd_rn(accf[j][k][h], __uint_as_float(w0[q][h])),
+                                                              __uint_as_float(w1[q][h]));
                                 }
-                                acc[j][k][h][kNAcc - 1] = acc[j][k][h][kNAcc - 1] + odd_bytes(w0[h]) + odd_bytes(w1[h]);
-                            } else if constexpr (KIND == kKindU16) {
-                                acc[j][k][h][0] = acc[j][k][h][0] + w0[h] + w1[h];
-                            } else {                      // ascending channel order, one rounding per add
-                                accf[j][k][h] = __fadd_rn(__fadd_rn(accf[j][k][h], __uint_as_float(w0[h])),
-                                                          __uint_as_float(w1[h]));
                             }
                         }
                     }
