@@ -235,10 +235,6 @@ __global__ void __launch_bounds__(kThreads, 1) ddsp_lanes_kernel(const LanesArgs
                         for (int e = 0; e < kNAcc; ++e) acc[j][k][h][e] = 0u;
                 }
 
-        // 16-bit lanes -> output rows (uint8 kinds); fp32 accumulators -> output rows (float32, once)
-        // 16-bit lanes -> uint32 output rows (first flush of the item: store; later: reduction); fp32 accumulators ->
-        // output rows, once.  Column offsets are 32-bit (W * Q < 2^31, checked at launch).  The common case -- a real
-        // trial, every column of this thread inside [0, nout) -- runs without a per-element test.
         bool first_flush = true;
         // FIRST: plain stores, else reductions; CHECKED: test every column against the end of the output
         auto flush_body = [&](auto first_tag, auto checked_tag) {
