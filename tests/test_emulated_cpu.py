@@ -338,3 +338,18 @@ def test_lanes_random_plans(emu, oracle):
         if done == 12:
             break
     assert done == 12
+
+
+@pytest.mark.parametrize("name", ["fast", "wide", "lowfreq", "rfids"])
+def test_lanes_all_channels_last_dm_block(emu, oracle, name):
+    """The big configs with ALL their channels (e.g. `fast`: 512 chunks through a ring of 5 stages, 8 flushes of
+    the 16-bit lanes; `rfids`: mask, x4 bins, 29 flushes; the longest windows of each plan) for the last, ragged
+    block of DM trials, cropped to one time tile."""
+    full = synth.config(name)
+    dms = full.dm_list[-9:]
+    wl = synth.Workload(name + "-allchan", full.seed, full.nchan, full.f_top, full.chan_bw, full.tsamp, 1, dms,
+                        downsample=full.downsample, dtype=full.dtype, mean=full.mean, std=full.std)
+    wl.mask = full.mask
+    _, dmax = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, wl.downsample)
+    wl = wl.cropped(wl.downsample * (dmax + 333) - (2 if wl.downsample > 1 else 0))
+    check(emu, oracle, wl, LANES)
