@@ -1,4 +1,5 @@
-// ddsp_tiled.cu -- DDSP_KERNEL_TILED: shared-memory tiled brute-force dedispersion.
+// ddsp_tiled.cu -- DDSP_KERNEL_TILED: shared-memory tiled brute-force dedispersion, rows staged through registers
+// (the round-1 kernel, the one with a hardware history).
 //
 //   D[i][t] = sum over unmasked c of x[c][t + d(i,c)]
 //
@@ -17,9 +18,7 @@
 // flushed to the uint32 output rows (global memory, L2-resident, owned by this thread) every 256
 // channels (255 * 257 < 65536).
 //
-// float32 path.  One staged copy (4-byte elements are always aligned); one fp32 register accumulator
-// per output element, channels added in ascending order with __fadd_rn: bit-identical to the
-// sequential sum (R9).  With ds > 1 the bins ((x0 + x1) + x2) + ... are formed at staging.
+// uint8 input with ds = 1 only; everything else runs on the lanes kernels (ddsp_lanes.cu) or the direct kernel.
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
