@@ -1,6 +1,6 @@
 """Build libddsp.so (the C-ABI library of include/ddsp.h) in-tree with nvcc for sm_100a.
 
-    python -m paper_2511_02328_b200.build [--force] [--verbose]
+    python -m paper_2511_02328_b200.build [--force] [--verbose] [--define NAME=VALUE ...]
 
 nvcc cross-compiles without a GPU.  The .so lands next to this file so that it travels with the
 repository snapshot to the GPU box; it is git-ignored.
@@ -40,9 +40,10 @@ def _stale():
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False):
-    """Compile every CUDA source into libddsp.so; returns its path."""
-    if not force and not _stale():
+def build(force=False, verbose=False, defines=()):
+    """Compile every CUDA source into libddsp.so; returns its path.  defines: compile-time tuning knobs
+    ("NAME=VALUE", see csrc/ddsp_lanes.cu); a build with defines is always redone and is not what ships."""
+    if not force and not defines and not _stale():
         return LIB
     objs = []
     bdir = os.path.join(_HERE, "build")
@@ -50,7 +51,7 @@ def build(force=False, verbose=False):
     procs = []
     for s in SOURCES:
         o = os.path.join(bdir, os.path.splitext(s)[0] + ".o")
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-D" + d for d in defines] + \
               ["-c", os.path.join(CSRC, s), "-o", o]
         procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT)))
         objs.append(o)
@@ -67,4 +68,5 @@ def build(force=False, verbose=False):
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    defs = [sys.argv[i + 1] for i, a in enumerate(sys.argv[:-1]) if a == "--define"]
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, defines=defs))

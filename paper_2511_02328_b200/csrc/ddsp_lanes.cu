@@ -47,14 +47,27 @@ namespace {
 // ------------------------------------------------------------------------------------------------
 // compile-time geometry
 // ------------------------------------------------------------------------------------------------
-constexpr int kBDM = 16;                        // trials per work item
+// Compile-time tuning knobs (build.py --define NAME=VALUE); the defaults are what ships.  kSlabs * kGroups = 16
+// warps always; (slabs, groups) = (4, 4): 16 trials x 512 words per item; (2, 8): 32 trials x 256 words (half the
+// passes over the interleaved copy, windows twice as long).
+#ifndef DDSP_LANES_SLABS
+#define DDSP_LANES_SLABS 4
+#endif
+#ifndef DDSP_LANES_GROUPS
+#define DDSP_LANES_GROUPS 4
+#endif
+#ifndef DDSP_LANES_FMA_E
+#define DDSP_LANES_FMA_E 1                     // uint8: whole-word adds as IMAD (FMA pipe); 0: IADD3 (ALU pipe)
+#endif
 constexpr int kDT = 4;                          // trials per thread
 constexpr int kMW = 4;                          // words per thread per trial, strided by 32 lanes
-constexpr int kSlabs = 4;                       // slabs of kMW * 32 = 128 words
-constexpr int kGroups = kBDM / kDT;             // trial groups
+constexpr int kSlabs = DDSP_LANES_SLABS;        // slabs of kMW * 32 = 128 words
+constexpr int kGroups = DDSP_LANES_GROUPS;      // trial groups
+constexpr int kBDM = kGroups * kDT;             // trials per work item
 constexpr int kWarps = kSlabs * kGroups;        // 16
 constexpr int kThreads = 32 * kWarps;           // 512
-constexpr int kTW = kSlabs * kMW * 32;          // 512 words per work item
+constexpr int kTW = kSlabs * kMW * 32;          // words per work item
+static_assert(kWarps == 16, "512 threads x 128 registers = the register file");
 constexpr int kC = 4;                           // channel rows per chunk (one ring stage)
 constexpr int kTblWords = kC * kBDM;            // per-chunk table: shared-memory offset of every (row, trial)
 constexpr int kTblBytes = kTblWords * 4;
@@ -406,7 +419,7 @@ typedef void (*PreKernel)(const PreArgs);
 typedef void (*LanesKernel)(const LanesArgs);
 const PreKernel kPreKernels[3] = {ddsp_interleave_kernel<kKindU8>, ddsp_interleave_kernel<kKindU16>,
                                   ddsp_interleave_kernel<kKindF32>};
-const LanesKernel kLanesKernels[3] = {ddsp_lanes_kernel<kKindU8, 1>, ddsp_lanes_kernel<kKindU16, 0>,
+const LanesKernel kLanesKernels[3] = {ddsp_lanes_kernel<kKindU8, DDSP_LANES_FMA_E>, ddsp_lanes_kernel<kKindU16, 0>,
                                       ddsp_lanes_kernel<kKindF32, 0>};
 const int kWordBytes[3] = {Kind<kKindU8>::WB, Kind<kKindU16>::WB, Kind<kKindF32>::WB};
 const int kLanesPerWord[3] = {Kind<kKindU8>::W, Kind<kKindU16>::W, Kind<kKindF32>::W};

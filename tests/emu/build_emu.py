@@ -42,11 +42,14 @@ def _stale(target, deps):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(tsan=False, mutate=None):
+def build(tsan=False, mutate=None, defines=()):
     """mutate = (name, old, new): build emu_tsan_<name> with `old` replaced by `new` in the kernel sources --
     a deliberately broken protocol, to show that the race check can fail (negative control)."""
     os.makedirs(BUILD, exist_ok=True)
     target = TSAN_EXE if tsan else LIB
+    if defines:         # a tuning-knob build (csrc/ddsp_lanes.cu): its own library
+        assert not tsan and not mutate
+        target = LIB.replace(".so", "_" + "_".join(d.replace("=", "") for d in defines) + ".so")
     if mutate:
         assert tsan
         target = TSAN_EXE + "_" + mutate[0]
@@ -70,7 +73,7 @@ def build(tsan=False, mutate=None):
             f.write(text)
         srcs.append(out)
     srcs += [os.path.join(HERE, "emu_runtime.cpp")]
-    flags = ["-std=c++17", "-O1", "-g", "-fPIC", "-pthread", "-ffp-contract=off", "-fno-fast-math", "-w", "-DDDSP_TESTING",
+    flags = ["-std=c++17", "-O1", "-g", "-fPIC", "-pthread", "-ffp-contract=off", "-fno-fast-math", "-w", "-DDDSP_TESTING"] + ["-D" + d for d in defines] + [
              "-I", HERE, "-I", CSRC, "-I", os.path.join(ROOT, "include")]
     if tsan:
         cmd = ["g++"] + flags + ["-fsanitize=thread"] + srcs + [os.path.join(HERE, "emu_tsan_main.cpp"), "-o", target]

@@ -353,3 +353,23 @@ def test_lanes_all_channels_last_dm_block(emu, oracle, name):
     _, dmax = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, wl.downsample)
     wl = wl.cropped(wl.downsample * (dmax + 333) - (2 if wl.downsample > 1 else 0))
     check(emu, oracle, wl, LANES)
+
+
+# ---- compile-time tuning knobs (csrc/ddsp_lanes.cu): the alternative geometries are correct too ------------------
+@pytest.mark.parametrize("defines", [("DDSP_LANES_SLABS=2", "DDSP_LANES_GROUPS=8"), ("DDSP_LANES_FMA_E=0",),
+                                     ("DDSP_LANES_SLABS=8", "DDSP_LANES_GROUPS=2")])
+def test_lanes_tuning_knobs(oracle, defines):
+    """32 trials x 256 words per item (and 8 x 1024), and the all-ALU accumulate: same results, same range checks."""
+    lib = ctypes.CDLL(build_emu.build(defines=defines))
+    for name, (res, args) in binding.SIGNATURES.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    lib.ddsp_emu_faults.restype = ctypes.c_long
+    lib.ddsp_emu_register.argtypes = [ctypes.c_void_p, ctypes.c_size_t]
+    lib.ddsp_emu_unregister.argtypes = [ctypes.c_void_p]
+    check(lib, oracle, small(mask_frac=0.2, ndm=37, nsamp=2100), LANES)
+    check(lib, oracle, small(ds=4, nsamp=4 * 1500 + 3, dm_max=160.0, ndm=33), LANES)
+    check(lib, oracle, small(dtype="f32", nsamp=1300, dm_max=30.0, ndm=33), LANES)
+    wl = small(nchan=261, nsamp=900, ndm=35, dm_max=6.0, seed=5)      # several flushes, ragged last DM block
+    wl.chan_bw = -0.5
+    check(lib, oracle, wl, LANES)
