@@ -281,12 +281,20 @@ def test_negative_control_input_too_small(emu, oracle):
 
 
 # ---- race check of the shared-memory protocol under ThreadSanitizer (tests/emu/emu_tsan_main.cpp) -------------
-def _run_tsan(exe, case, halt=0):
+def _run_tsan(exe, case, halt=0, timeout=900):
+    """Returns (returncode or None if it had to be killed, stdout, stderr)."""
     env = dict(os.environ, TSAN_OPTIONS="halt_on_error=%d report_signal_unsafe=0" % halt)
-    r = subprocess.run([exe, case], capture_output=True, text=True, timeout=900, env=env)
-    if "FATAL: ThreadSanitizer" in r.stderr:        # e.g. an address-space layout the sanitizer runtime rejects
-        pytest.skip("ThreadSanitizer cannot run here: " + r.stderr.strip().splitlines()[0])
-    return r
+    p = subprocess.Popen([exe, case], stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, env=env)
+    try:
+        out, err = p.communicate(timeout=timeout)
+        rc = p.returncode
+    except subprocess.TimeoutExpired:
+        p.kill()
+        out, err = p.communicate()
+        rc = None
+    if "FATAL: ThreadSanitizer" in err:        # e.g. an address-space layout the sanitizer runtime rejects
+        pytest.skip("ThreadSanitizer cannot run here: " + err.strip().splitlines()[0])
+    return rc, out, err
 
 
 @pytest.mark.parametrize("case", ["u8", "bins2", "bins4", "f32"])
@@ -294,10 +302,10 @@ def test_lanes_protocol_is_race_free(case):
     """More chunks than ring stages and several work items per CTA, so every stage is refilled by the copy engine
     while other warps are still at work on its neighbours: no shared-memory access may be unordered with
     respect to the copy engine."""
-    r = _run_tsan(build_emu.build(tsan=True), case)
-    assert "ThreadSanitizer" not in r.stderr, r.stderr[-3000:]
-    assert r.returncode == 0, (r.stdout, r.stderr[-2000:])
-    assert "faults=0" in r.stdout and "status=0" in r.stdout
+    rc, out, err = _run_tsan(build_emu.build(tsan=True), case)
+    assert "ThreadSanitizer" not in err, err[-3000:]
+    assert rc == 0, (rc, out, err[-2000:])
+    assert "faults=0" in out and "status=0" in out
 
 
 def test_lanes_race_check_can_fail():
@@ -305,8 +313,13 @@ def test_lanes_race_check_can_fail():
     reported as a data race -- otherwise the clean runs above would prove nothing."""
     exe = build_emu.build(tsan=True, mutate=("early", "if (p_issued >= a.NS) ok = mbar_wait(", "if (false) ok = mbar_wait(",
                                               "ddsp_lanes.cu"))
-    r = _run_tsan(exe, "u8", halt=1)          # the first report ends the run
-    assert "ThreadSanitizer: data race" in r.stderr
+    # The broken protocol may also lose a barrier phase and sit in its bounded waits; all that matters here is
+    # that the unordered access is reported, so the run is cut short.
+    for attempt in range(3):                  # thread interleavings differ from run to run
+        rc, out, err = _run_tsan(exe, "u8", halt=1, timeout=240)
+        if "ThreadSanitizer: data race" in err:
+            break
+    assert "ThreadSanitizer: data race" in err, (rc, out, err[-1500:])
 
 
 # ---- seeded random plans: whatever the shape, the lanes kernels equal the oracle and stay inside their buffers -----
