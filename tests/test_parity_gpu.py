@@ -340,3 +340,19 @@ def test_full_size_fast_first_and_last_columns(oracle, kernel):
             got = to_host(out, plan, rows, c0, c0 + ncol)
             assert_u32_equal(got, want, "fast full size, columns from %d" % c0)
         assert bool((out[:, nout:] == -7).all()), "pitch padding was written"
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_dm_row_split_is_a_row_range(oracle, kernel):
+    """ddsp_plan_create_rows: the outputs of plans that split one DM list are the row ranges of
+    the whole list's output, with the whole list's nsamp_out (invariant I7)."""
+    wl = _small(ndm=45, dm_max=80.0, nsamp=6000)
+    x = make_input(oracle, wl, "cuda")
+    want, nout, _ = oracle.dedisperse(x.cpu().numpy(), wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list)
+    for begin, count in ((0, 23), (23, 22), (40, 5)):
+        with binding.plan_for(wl, rows=(begin, count)) as plan:
+            _set_kernel(plan, kernel)
+            assert plan.nsamp_out == nout and plan.ndm == count
+            out = run_plan(plan, x)
+            assert plan.device_status() == 0
+            assert_u32_equal(to_host(out, plan), want[begin:begin + count], "rows %d+%d" % (begin, count))
