@@ -149,6 +149,15 @@ def config(name):
         return _finish(Workload("rfids", 4, 2048, 1500.0, -0.244140625, 49.152e-6, 3051758,
                                 np.arange(0, 2001, dtype=np.float64), downsample=4,
                                 n_rfi=8, n_zap=205, n_spikes=3))
+    # Context sweeps shaped like the paper's E1 / E2 timing experiments (synthetic 8-bit data,
+    # 22 s at 40 us, 1000-1500 MHz, DM 0-1024; E1: 1500 trials, channels swept; E2: 2048 channels, trials swept).
+    # Not BASELINE.json configs and not targets: `bench.py --config e1:4096` / `e2:8192` give numbers to set
+    # beside the paper's RTX 4090 figures.
+    if isinstance(name, str) and name[:3] in ("e1:", "e2:"):
+        n = int(name[3:])
+        nchan, ndm = (n, 1500) if name[:2] == "e1" else (2048, n)
+        return _finish(Workload(name, 10 + n % 97, nchan, 1500.0, -500.0 / nchan, 40e-6, 550000,
+                                np.linspace(0.0, 1024.0, ndm)))
     raise KeyError(name)
 
 
