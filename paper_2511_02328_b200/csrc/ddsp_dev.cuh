@@ -82,9 +82,18 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 // ---- global memory -----------------------------------------------------------------------------------------
 __device__ __forceinline__ void st_global_u32(uint32_t* p, uint32_t v) { *p = v; }
 __device__ __forceinline__ void st_global_f32(float* p, float v) { *p = v; }
-// *p += v without a return value (SASS RED): the issuing thread does not wait for the result
+// *p += v on an element that only this thread ever touches.  Default: a reduction store (SASS RED: no return
+// value, the issuing thread does not wait).  -DDDSP_LANES_FLUSH_RMW=1: plain load / add / store instead (tuning
+// knob, in case the L2's atomic units turn out to be the narrower path).
+#ifndef DDSP_LANES_FLUSH_RMW
+#define DDSP_LANES_FLUSH_RMW 0
+#endif
 __device__ __forceinline__ void red_add_u32(uint32_t* p, uint32_t v) {
+#if DDSP_LANES_FLUSH_RMW
+    *p += v;
+#else
     asm volatile("red.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+#endif
 }
 __device__ __forceinline__ void report_status(int* status, int code) { atomicCAS(status, 0, code); }
 __device__ __forceinline__ uint32_t ldg_u8(const uint8_t* p) { return (uint32_t)__ldg(p); }
