@@ -508,6 +508,7 @@ int ddsp_lanes_plan(ddsp_plan* p) {
     int64_t NT, Q, M;
     ddsp_lanes_range(p, p->nsamp_out, &NT, &Q, &M);
     if ((int64_t)g.nblk * NT * std::max(g.nchunk, 1) >= ((int64_t)1 << 31)) return DDSP_OK;   // 32-bit chunk counters
+    if (Q * kLanesPerWord[g.kind] >= ((int64_t)1 << 31)) return DDSP_OK;                       // 32-bit column offsets
     g.ws_bytes = (size_t)std::max(nlist, 1) * (size_t)M * WB;
     g.ok = true;
     return DDSP_OK;

@@ -147,3 +147,17 @@ def test_plan_rows_is_a_row_range_of_the_whole_plan(lib, oracle):
     for bad in ((-1, 5), (0, 0), (200, 2), (201, 1)):
         with pytest.raises(binding.DdspError):
             binding.plan_for(wl, rows=bad)
+
+
+def test_lanes_declines_what_its_32_bit_counters_cannot_hold(lib):
+    """More than 2**31 output columns: the lanes kernels say UNSUPPORTED at plan time (AUTO falls back), they do not
+    fail at launch."""
+    with binding.Plan(2, 1500.0, -10.0, 1e-3, 3 * 2 ** 30, [0.0, 1.0]) as plan:
+        with pytest.raises(binding.DdspError) as ei:
+            plan.set_kernel(binding.DDSP_KERNEL_LANES)
+        assert ei.value.code == binding.DDSP_ERR_UNSUPPORTED
+        assert plan.kernel in (binding.DDSP_KERNEL_DIRECT, binding.DDSP_KERNEL_TILED)
+    with binding.Plan(2, 1500.0, -10.0, 1e-3, 2 ** 20, [0.0, 1.0]) as plan:
+        plan.set_kernel(binding.DDSP_KERNEL_LANES)          # host-only plan: geometry exists, nothing is allocated
+        assert plan.kernel == binding.DDSP_KERNEL_LANES and plan.workspace_bytes > 0
+        assert plan.launches_per_execute == 2
