@@ -220,7 +220,9 @@ def test_I5_masked_channels_never_read(oracle, kernel):
         x = make_input(oracle, wl, "cuda")
         with binding.plan_for(wl) as plan:
             _set_kernel(plan, kernel)
-            ref = to_host(run_plan(plan, x), plan)
+            out = run_plan(plan, x)
+            ref = to_host(out, plan)
+            _compare(oracle, wl, plan, x, out, what="I5 reference " + dtype)      # the reference itself is the oracle's
             x2 = x.clone()
             zap = torch.as_tensor(np.flatnonzero(wl.mask), device="cuda")
             x2[zap] = float("nan") if dtype == "f32" else 255
