@@ -56,6 +56,9 @@ namespace {
 #ifndef DDSP_LANES_GROUPS
 #define DDSP_LANES_GROUPS 4
 #endif
+#ifndef DDSP_LANES_ROWS
+#define DDSP_LANES_ROWS 4                      // channel rows per chunk (ring stage); even; 6 or 8 trade ring depth for
+#endif                                         // fewer barrier rounds per row
 #ifndef DDSP_LANES_FMA_E
 #define DDSP_LANES_FMA_E 1                     // uint8: whole-word adds as IMAD (FMA pipe); 0: IADD3 (ALU pipe)
 #endif
@@ -68,7 +71,8 @@ constexpr int kWarps = kSlabs * kGroups;        // 16
 constexpr int kThreads = 32 * kWarps;           // 512
 constexpr int kTW = kSlabs * kMW * 32;          // words per work item
 static_assert(kWarps == 16, "512 threads x 128 registers = the register file");
-constexpr int kC = 4;                           // channel rows per chunk (one ring stage)
+constexpr int kC = DDSP_LANES_ROWS;              // channel rows per chunk (one ring stage)
+static_assert(kC >= 2 && kC % 2 == 0 && kC <= 16, "rows per chunk: even, producer lanes 0..kC");
 constexpr int kTblWords = kC * kBDM;            // per-chunk table: shared-memory offset of every (row, trial)
 constexpr int kTblBytes = kTblWords * 4;
 constexpr int kBarBytes = 1024;                 // mbarriers and the abort flag live in the first 1 KB

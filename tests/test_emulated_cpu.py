@@ -370,7 +370,8 @@ def test_lanes_all_channels_last_dm_block(emu, oracle, name):
 
 # ---- compile-time tuning knobs (csrc/ddsp_lanes.cu): the alternative geometries are correct too ------------------
 @pytest.mark.parametrize("defines", [("DDSP_LANES_SLABS=2", "DDSP_LANES_GROUPS=8"), ("DDSP_LANES_FMA_E=0",),
-                                     ("DDSP_LANES_SLABS=8", "DDSP_LANES_GROUPS=2")])
+                                     ("DDSP_LANES_SLABS=8", "DDSP_LANES_GROUPS=2"), ("DDSP_LANES_ROWS=6",),
+                                     ("DDSP_LANES_ROWS=8", "DDSP_LANES_FLUSH_RMW=1")])
 def test_lanes_tuning_knobs(oracle, defines):
     """32 trials x 256 words per item (and 8 x 1024), and the all-ALU accumulate: same results, same range checks."""
     lib = ctypes.CDLL(build_emu.build(defines=defines))
