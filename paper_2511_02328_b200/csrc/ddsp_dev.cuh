@@ -95,6 +95,9 @@ __device__ __forceinline__ void red_add_u32(uint32_t* p, uint32_t v) {
     asm volatile("red.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 #endif
 }
+// plain loads / stores of output elements: named so that the CPU emulation can range-check them
+__device__ __forceinline__ uint32_t ld_global_u32(const uint32_t* p) { return *p; }
+__device__ __forceinline__ uint4 ld_global_v4(const void* p) { return *reinterpret_cast<const uint4*>(p); }
 __device__ __forceinline__ void report_status(int* status, int code) { atomicCAS(status, 0, code); }
 __device__ __forceinline__ uint32_t ldg_u8(const uint8_t* p) { return (uint32_t)__ldg(p); }
 __device__ __forceinline__ float ldg_f32(const float* p) { return __ldg(p); }

@@ -8,6 +8,7 @@
 // channel row (coalesced); the delay d(i,c) is uniform over the block.  All element offsets are 64-bit
 // (config 2's input is 6.25e9 bytes).
 #include "ddsp_internal.h"
+#include "ddsp_dev.cuh"
 
 namespace {
 
@@ -44,6 +45,8 @@ __device__ __forceinline__ float bin_sum<float, float>(const float* __restrict__
     return s;
 }
 
+__device__ __forceinline__ void store_out(uint32_t* p, uint32_t v) { ddsp_dev::st_global_u32(p, v); }
+__device__ __forceinline__ void store_out(float* p, float v) { ddsp_dev::st_global_f32(p, v); }
 __device__ __forceinline__ void accumulate(uint32_t& acc, uint32_t v) { acc += v; }
 __device__ __forceinline__ void accumulate(float& acc, float v) { acc = __fadd_rn(acc, v); }  // never an FMA
 
@@ -77,7 +80,7 @@ ddsp_direct_kernel(const TIn* __restrict__ in, TAcc* __restrict__ out, const int
 #pragma unroll
     for (int k = 0; k < kPerThread; ++k) {
         const int64_t t = t0 + (int64_t)k * kThreads;
-        if (t < nsamp_out) orow[t] = acc[k];
+        if (t < nsamp_out) store_out(orow + t, acc[k]);
     }
     }
 }

@@ -182,15 +182,15 @@ __global__ void __launch_bounds__(128 * GROUPS, 1) ddsp_tiled_u8_kernel(const Ti
                 uint32_t v0 = e & 0xffffu, v2 = e >> 16, v1 = o & 0xffffu, v3 = o >> 16;
                 if (a.out_vec && t + 3 < a.nsamp_out) {
                     if (!first_flush) {
-                        const uint4 old = *reinterpret_cast<const uint4*>(p);
+                        const uint4 old = ld_global_v4(p);
                         v0 += old.x; v1 += old.y; v2 += old.z; v3 += old.w;
                     }
-                    *reinterpret_cast<uint4*>(p) = make_uint4(v0, v1, v2, v3);
+                    st_global_v4(p, v0, v1, v2, v3);
                 } else {
                     const uint32_t v[4] = {v0, v1, v2, v3};
 #pragma unroll
                     for (int s = 0; s < 4; ++s)
-                        if (t + s < a.nsamp_out) p[s] = first_flush ? v[s] : p[s] + v[s];
+                        if (t + s < a.nsamp_out) st_global_u32(p + s, first_flush ? v[s] : ld_global_u32(p + s) + v[s]);
                 }
             }
         }

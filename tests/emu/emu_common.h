@@ -62,6 +62,14 @@ inline void fence_proxy_async_smem() {}
 inline void st_global_u32(uint32_t* p, uint32_t v) { emu::check_global(p, 4, true); *p = v; }
 inline void st_global_f32(float* p, float v) { emu::check_global(p, 4, true); *p = v; }
 inline void red_add_u32(uint32_t* p, uint32_t v) { emu::check_global(p, 4, true); __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+inline uint32_t ld_global_u32(const uint32_t* p) { emu::check_global(p, 4, false); return *p; }
+inline uint4 ld_global_v4(const void* p) {
+    emu::check_global(p, 16, false);
+    emu::check_aligned(p, 16);
+    uint4 v;
+    std::memcpy(&v, p, 16);
+    return v;
+}
 inline void report_status(int* status, int code) {
     emu::check_global(status, 4, true);
     int zero = 0;

@@ -201,14 +201,15 @@ def test_lanes_unaligned_dense_input(emu, oracle, dtype, ds):
     check(emu, oracle, wl, LANES, misalign=4 if dtype == "f32" else 3)
 
 
+@pytest.mark.parametrize("kernel", [LANES, TILED, DIRECT], ids=["lanes", "tiled", "direct"])
 @pytest.mark.parametrize("name,extra", [("fast", 700), ("wide", 600), ("lowfreq", 500), ("rfids", 650)])
-def test_lanes_real_geometries_cropped(emu, oracle, name, extra):
+def test_real_geometries_cropped(emu, oracle, name, extra, kernel):
     """The real configs' channel grids and DM steps (so the real window lengths, ring depth and stage sizes),
-    cropped in time and thinned in DM blocks: first, middle and last block of 16 trials."""
+    cropped in time and thinned in DM blocks: first, middle and last block of 32 trials."""
     full = synth.config(name)
-    nblk = (full.ndm + 15) // 16
+    nblk = (full.ndm + 31) // 32                      # blocks of 32: whole blocks for the tiled kernel, pairs for lanes
     blocks = sorted({0, nblk // 2, nblk - 1})
-    dms = np.concatenate([full.dm_list[16 * b:16 * b + 16] for b in blocks])
+    dms = np.concatenate([full.dm_list[32 * b:32 * b + 32] for b in blocks])
     # every 16th channel keeps the band, the delay spread per trial and the run time of the emulation small
     sub = slice(None, None, 16)
     wl = synth.Workload(name + "-emu", full.seed, len(np.arange(full.nchan)[sub]), full.f_top, full.chan_bw * 16,
@@ -216,7 +217,9 @@ def test_lanes_real_geometries_cropped(emu, oracle, name, extra):
                         std=full.std)
     _, dmax = oracle.delay_table(wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.dm_list, wl.downsample)
     wl = wl.cropped(wl.downsample * (dmax + extra) - (1 if wl.downsample > 1 else 0))
-    check(emu, oracle, wl, LANES)
+    if kernel == TILED:      # 2048 outputs per tile: a full tile plus a ragged one, dense rows of odd pitch as well
+        wl = wl.cropped(wl.nsamp + 2048 + 37)
+    check(emu, oracle, wl, kernel)
 
 
 @pytest.mark.parametrize("kind,pieces", [("u8", 3), ("u8", 7), ("bins4", 3), ("f32", 2)])
@@ -252,6 +255,32 @@ def test_negative_control_output_too_small(emu, oracle):
         f0 = emu.ddsp_emu_faults()
         assert emu.ddsp_execute(h, xin.a.ctypes.data, out.ctypes.data, None) == 0
         assert emu.ddsp_emu_faults() - f0 == 4
+        emu.ddsp_emu_unregister(out.ctypes.data)
+        xin.release()
+    finally:
+        emu.ddsp_plan_destroy(h)
+
+
+@pytest.mark.parametrize("kernel", [TILED, DIRECT], ids=["tiled", "direct"])
+def test_negative_control_output_too_small_other_kernels(emu, oracle, kernel):
+    """The same for the kernels with a hardware history: their output stores and read-modify-write flushes go
+    through range-checked helpers too."""
+    wl = small()
+    x = host_input(wl)
+    dm = np.ascontiguousarray(wl.dm_list, dtype=np.float64)
+    h = ctypes.c_void_p()
+    assert emu.ddsp_plan_create(ctypes.byref(h), wl.nchan, wl.f_top, wl.chan_bw, wl.tsamp, wl.nsamp, dm.ctypes.data,
+                                dm.size, 1, None, binding.DDSP_IN_U8) == 0
+    try:
+        nout = emu.ddsp_plan_nsamp_out(h)
+        assert emu.ddsp_plan_set_kernel(h, kernel) == 0
+        xin = DeviceArray(emu, x.shape, x.dtype)
+        xin.a[...] = x
+        out = np.zeros((wl.ndm, nout), dtype=np.uint32)
+        emu.ddsp_emu_register(out.ctypes.data, out.nbytes - 16)
+        f0 = emu.ddsp_emu_faults()
+        assert emu.ddsp_execute(h, xin.a.ctypes.data, out.ctypes.data, None) == 0
+        assert emu.ddsp_emu_faults() - f0 >= 1
         emu.ddsp_emu_unregister(out.ctypes.data)
         xin.release()
     finally:
